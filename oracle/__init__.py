@@ -1,0 +1,104 @@
+"""CPU oracle for arxiv 1501.03869 (FMM + Eq. 7 back projection).
+
+TEST INFRASTRUCTURE ONLY: importable from tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs, never from the product
+package.  Thin ctypes marshalling over oracle/pat_oracle.c; no arithmetic of
+the method lives in this file.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from .build import build as _build
+
+_lib = None
+
+# (wp, wd) of  b = wp*p - wd*t*dp/dt  (Eq. 7; reading R1)
+WEIGHTS = {0: (1.0, 0.0), 1: (1.0, 1.0), 2: (2.0, 2.0)}
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(_build())
+        i32, i64, f32, f64 = ctypes.c_int32, ctypes.c_int64, ctypes.c_float, ctypes.c_double
+        vp = ctypes.c_void_p
+        L.oracle_fmm.restype = ctypes.c_int
+        L.oracle_fmm.argtypes = [i32, vp, f64, vp, vp, vp, i32, vp, vp]
+        L.oracle_fmm_rows.restype = ctypes.c_int
+        L.oracle_fmm_rows.argtypes = [i32, vp, f64, vp, vp, vp, i32, vp, i64, i32, vp]
+        L.oracle_weight.restype = None
+        L.oracle_weight.argtypes = [vp, i32, f64, f64, f64, vp]
+        L.oracle_backproject.restype = ctypes.c_int
+        L.oracle_backproject.argtypes = [vp, i64, vp, i32, i64, i32, i32, f32, f32, f64, f64, vp]
+        _lib = L
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def fmm(n, h, origin, c_map, src, order=1, return_order=False):
+    """Arrival times (double, shape n[::-1]) from a point source."""
+    ndim = len(n)
+    n3 = np.array(list(n) + [1] * (3 - ndim), dtype=np.int32)
+    org = np.array(list(origin) + [0.0] * (3 - len(origin)), dtype=np.float64)
+    s = np.array(list(src) + [0.0] * (3 - len(src)), dtype=np.float64)
+    c = np.ascontiguousarray(c_map, dtype=np.float32).ravel()
+    N = int(np.prod(n3))
+    assert c.size == N
+    T = np.empty(N, dtype=np.float64)
+    fo = np.full(N, -1, dtype=np.int64) if return_order else None
+    rc = lib().oracle_fmm(ndim, _p(n3), float(h), _p(org), _p(c), _p(s), int(order), _p(T),
+                          _p(fo) if fo is not None else None)
+    if rc:
+        raise ValueError("oracle_fmm failed with code %d" % rc)
+    T = T.reshape(tuple(int(v) for v in n3[:ndim][::-1]))
+    return (T, fo) if return_order else T
+
+
+def fmm_rows(n, h, origin, c_map, sensors, roi_index, order=1):
+    """tau[i][j] fp32 = arrival time sensor i -> ROI node j (reciprocity)."""
+    ndim = len(n)
+    n3 = np.array(list(n) + [1] * (3 - ndim), dtype=np.int32)
+    org = np.array(list(origin) + [0.0] * (3 - len(origin)), dtype=np.float64)
+    c = np.ascontiguousarray(c_map, dtype=np.float32).ravel()
+    sens = np.ascontiguousarray(sensors, dtype=np.float64).reshape(-1, 3)
+    roi = np.ascontiguousarray(roi_index, dtype=np.int64)
+    tau = np.empty((sens.shape[0], roi.size), dtype=np.float32)
+    rc = lib().oracle_fmm_rows(ndim, _p(n3), float(h), _p(org), _p(c), _p(sens), sens.shape[0],
+                               _p(roi), roi.size, int(order), _p(tau))
+    if rc:
+        raise ValueError("oracle_fmm_rows failed with code %d" % rc)
+    return tau
+
+
+def weight(p, mode=1, t0fs=0.0):
+    """b[n] = wp*p[n] - wd*(n + t0*fs)*D[n] in double."""
+    p = np.ascontiguousarray(p, dtype=np.float32)
+    b = np.empty(p.size, dtype=np.float64)
+    wp, wd = WEIGHTS[mode]
+    lib().oracle_weight(_p(p), p.size, wp, wd, float(t0fs), _p(b))
+    return b
+
+
+def backproject(tau, traces, fs, t0=0.0, mode=1):
+    """Eq. 7 image, double [nframes][npix]; tau fp32 [nsens][npix], traces fp32 [B][S][Nt]."""
+    tau = np.asarray(tau)
+    assert tau.dtype == np.float32 and tau.ndim == 2 and tau.strides[1] == 4
+    traces = np.ascontiguousarray(traces, dtype=np.float32)
+    if traces.ndim == 2:
+        traces = traces[None]
+    B, S, Nt = traces.shape
+    assert tau.shape[0] == S
+    P = tau.shape[1]
+    pitch = tau.strides[0] // 4 if S > 1 else P
+    img = np.zeros((B, P), dtype=np.float64)
+    wp, wd = WEIGHTS[mode]
+    rc = lib().oracle_backproject(_p(tau), pitch, _p(traces), S, P, Nt, B,
+                                  float(np.float32(fs)), float(np.float32(t0)), wp, wd, _p(img))
+    if rc:
+        raise ValueError("oracle_backproject failed with code %d" % rc)
+    return img

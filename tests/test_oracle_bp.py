@@ -1,0 +1,228 @@
+"""Pins P6-P14 for oracle_weight / oracle_backproject (Eq. 7)."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as W
+
+FS = 20e6
+
+
+def _rand_case(rng, S=6, P=50, Nt=64, B=2, umax=None):
+    umax = umax or (Nt - 2)
+    tau = (rng.uniform(0.5, umax, size=(S, P)) / FS).astype(np.float32)
+    tr = rng.standard_normal((B, S, Nt)).astype(np.float32)
+    return tau, tr
+
+
+def _u(tau, fs=FS):
+    return (tau.astype(np.float32) * np.float32(fs)).astype(np.float32)
+
+
+# ---- P14: brute force, independent pure-Python float64 loops of Eq. 7 + weighting ----------
+def _brute(tau, tr, fs, mode):
+    wp, wd = {0: (1, 0), 1: (1, 1), 2: (2, 2)}[mode]
+    B, S, Nt = tr.shape
+    P = tau.shape[1]
+    img = np.zeros((B, P))
+    for f in range(B):
+        for j in range(P):
+            acc = 0.0
+            for i in range(S):
+                u = np.float32(tau[i, j]) * np.float32(fs)          # fp32 product
+                if not (u >= 0 and u < Nt - 1):
+                    continue
+                k = int(np.floor(u))
+                a = float(u) - k
+                vals = []
+                for n in (k, k + 1):
+                    p = tr[f, i].astype(np.float64)
+                    if n == 0:
+                        D = p[1] - p[0]
+                    elif n == Nt - 1:
+                        D = p[Nt - 1] - p[Nt - 2]
+                    else:
+                        D = (p[n + 1] - p[n - 1]) / 2
+                    vals.append(wp * p[n] - wd * n * D)
+                acc += (1 - a) * vals[0] + a * vals[1]
+            img[f, j] = acc
+    return img
+
+
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_p14_brute_force_tiny_grid(mode):
+    rng = np.random.default_rng(1)
+    tau, tr = _rand_case(rng, S=4, P=64, Nt=32, B=2, umax=33)   # some u beyond the record
+    tau[0, :5] = (np.array([0.0, 30.0, 30.999, 31.0, 0.25]) / FS).astype(np.float32)
+    got = oracle.backproject(tau, tr, FS, mode=mode)
+    np.testing.assert_allclose(got, _brute(tau, tr, FS, mode), rtol=1e-12, atol=1e-12)
+
+
+# ---- P7: conventional BP (analytic tau) + mode 0 = library np.interp ----------
+def test_p7_delay_and_sum_equals_np_interp():
+    g = W.make_geometry(0)
+    xy = g.roi_coords()
+    s = g.sensors.astype(np.float64)
+    dist = np.hypot(xy[None, :, 0] - s[:, None, 0], xy[None, :, 1] - s[:, None, 1])
+    tau = (dist / 1560.0).astype(np.float32)
+    rng = np.random.default_rng(3)
+    tr = rng.standard_normal((1, g.nsens, g.nt)).astype(np.float32)
+    got = oracle.backproject(tau, tr, g.fs, mode=0)[0]
+    u = _u(tau, g.fs).astype(np.float64)
+    assert not np.any(u == g.nt - 1)
+    ref = sum(np.interp(u[i], np.arange(g.nt), tr[0, i].astype(np.float64), left=0.0, right=0.0)
+              for i in range(g.nsens))
+    np.testing.assert_allclose(got, ref, rtol=1e-12, atol=1e-12)
+
+
+# ---- P8: linearity in the traces (north_star check 3) ----------------------------------------
+@pytest.mark.parametrize("mode", [0, 1])
+def test_p8_linearity(mode):
+    rng = np.random.default_rng(4)
+    tau, x = _rand_case(rng, S=8, P=100, Nt=128, B=1)
+    y = rng.standard_normal(x.shape).astype(np.float32)
+    al, be = 2.0, -0.5
+    # make the fp32 combination exact: x, y on a coarse dyadic grid
+    x = np.round(x * 256) / 256
+    y = np.round(y * 256) / 256
+    z = (al * x + be * y).astype(np.float32)
+    assert np.array_equal(z.astype(np.float64), al * x.astype(np.float64) + be * y.astype(np.float64))
+    bx = oracle.backproject(tau, x.astype(np.float32), FS, mode=mode)
+    by = oracle.backproject(tau, y.astype(np.float32), FS, mode=mode)
+    bz = oracle.backproject(tau, z, FS, mode=mode)
+    scale = np.max(np.abs(bz))
+    assert np.max(np.abs(bz - (al * bx + be * by))) <= 1e-12 * scale
+
+
+# ---- P9: closed forms -------------------------------------------------------------------------
+def test_p9_constant_signal_counts_valid_sensors():
+    rng = np.random.default_rng(5)
+    S, P, Nt = 7, 200, 64
+    tau = (rng.uniform(-10, Nt + 10, size=(S, P)) / FS).astype(np.float32)
+    tr = np.ones((1, S, Nt), np.float32)
+    u = _u(tau)
+    count = np.sum((u >= 0) & (u < Nt - 1), axis=0)
+    for mode in (0, 1):
+        got = oracle.backproject(tau, tr, FS, mode=mode)[0]
+        np.testing.assert_allclose(got, count, rtol=0, atol=1e-12)
+
+
+def test_p9_ramp_signal():
+    """p[n] = n: mode 0 image = sum_i u_ij; Eq. 7 annihilates signals linear in t."""
+    rng = np.random.default_rng(6)
+    S, P, Nt = 5, 120, 64
+    tau, _ = _rand_case(rng, S=S, P=P, Nt=Nt)
+    tr = np.tile(np.arange(Nt, dtype=np.float32), (1, S, 1))
+    u = _u(tau).astype(np.float64)
+    got0 = oracle.backproject(tau, tr, FS, mode=0)[0]
+    np.testing.assert_allclose(got0, u.sum(axis=0), rtol=1e-13)
+    got1 = oracle.backproject(tau, tr, FS, mode=1)[0]
+    np.testing.assert_allclose(got1, 0.0, atol=1e-10)
+
+
+def test_p9_quadratic_signal():
+    """p[n] = n^2: central differences exact => b[n] = -n^2, image = -sum(k^2 + a(2k+1))."""
+    rng = np.random.default_rng(7)
+    S, P, Nt = 5, 120, 64
+    tau, _ = _rand_case(rng, S=S, P=P, Nt=Nt, umax=Nt - 2.5)
+    tr = np.tile((np.arange(Nt, dtype=np.float64) ** 2).astype(np.float32), (1, S, 1))
+    u = _u(tau).astype(np.float64)
+    k = np.floor(u)
+    a = u - k
+    expect = -np.sum(k * k + a * (2 * k + 1), axis=0)
+    got = oracle.backproject(tau, tr, FS, mode=1)[0]
+    np.testing.assert_allclose(got, expect, rtol=1e-13)
+
+
+def test_weight_closed_forms_and_ends():
+    Nt = 16
+    n = np.arange(Nt, dtype=np.float64)
+    p = (3 * n * n - 2 * n + 5).astype(np.float32)
+    b = oracle.weight(p, mode=1)
+    D = 6 * n - 2
+    D[0] = p[1] - p[0]
+    D[-1] = p[-1] - p[-2]
+    np.testing.assert_allclose(b, p - n * D, rtol=1e-14)
+    np.testing.assert_array_equal(oracle.weight(p, mode=0), p.astype(np.float64))
+    np.testing.assert_array_equal(oracle.weight(p, mode=2), 2 * b)
+    # t0 shifts the time axis of the weight: t_n * fs = n + t0*fs
+    np.testing.assert_allclose(oracle.weight(p, mode=1, t0fs=2.5), p - (n + 2.5) * D, rtol=1e-14)
+
+
+# ---- P10: one sensor, delta trace => the linear-interpolation hat kernel --------------------
+def test_p10_hat_kernel():
+    Nt, n0 = 64, 20
+    uu = np.linspace(15, 25, 401)
+    tau = (uu / FS).astype(np.float32)[None, :]
+    tr = np.zeros((1, 1, Nt), np.float32)
+    tr[0, 0, n0] = 1.0
+    got = oracle.backproject(tau, tr, FS, mode=0)[0]
+    u = _u(tau)[0].astype(np.float64)
+    np.testing.assert_allclose(got, np.maximum(0, 1 - np.abs(u - n0)), atol=1e-14)
+
+
+# ---- P11 / P12: mode scaling, sensor permutation, batch = single frames ---------------------
+def test_p11_p12_modes_permutation_batch():
+    rng = np.random.default_rng(8)
+    tau, tr = _rand_case(rng, S=9, P=80, Nt=96, B=3)
+    i1 = oracle.backproject(tau, tr, FS, mode=1)
+    i2 = oracle.backproject(tau, tr, FS, mode=2)
+    np.testing.assert_array_equal(i2, 2 * i1)
+    perm = rng.permutation(9)
+    ip = oracle.backproject(np.ascontiguousarray(tau[perm]), np.ascontiguousarray(tr[:, perm]), FS, mode=1)
+    assert np.max(np.abs(ip - i1)) <= 1e-13 * np.max(np.abs(i1))
+    for f in range(3):
+        np.testing.assert_array_equal(oracle.backproject(tau, tr[f:f + 1], FS, mode=1)[0], i1[f])
+
+
+# ---- P13: tau outside the record / non-finite contributes 0 ---------------------------------
+def test_p13_out_of_record_and_nonfinite_tau():
+    rng = np.random.default_rng(9)
+    S, P, Nt = 4, 40, 32
+    tau, tr = _rand_case(rng, S=S, P=P, Nt=Nt, B=1)
+    base = oracle.backproject(tau[1:], tr[:, 1:], FS, mode=1)[0]
+    bad = np.array([np.inf, -np.inf, np.nan, -1e-9, (Nt - 1) / FS, 1.0, -3.0, 1e30], np.float32)
+    for v in bad:
+        t2 = tau.copy()
+        t2[0, :] = v
+        got = oracle.backproject(t2, tr, FS, mode=1)[0]
+        np.testing.assert_array_equal(got, base)
+    # u == 0 exactly is inside the record
+    t2 = tau.copy()
+    t2[0, :] = 0.0
+    got = oracle.backproject(t2, tr, FS, mode=0)[0]
+    np.testing.assert_allclose(got - oracle.backproject(tau[1:], tr[:, 1:], FS, mode=0)[0], tr[0, 0, 0], atol=1e-13)
+
+
+def test_t0_shifts_the_record():
+    rng = np.random.default_rng(10)
+    tau, tr = _rand_case(rng, S=3, P=30, Nt=64, B=1, umax=40)
+    t0 = np.float32(8) / np.float32(FS)
+    tau_shift = (tau + t0).astype(np.float32)
+    a = oracle.backproject(tau_shift, tr, FS, t0=float(t0), mode=0)
+    u = ((tau_shift - t0).astype(np.float32) * np.float32(FS)).astype(np.float64)
+    ref = sum(np.interp(u[i], np.arange(64), tr[0, i].astype(np.float64), left=0, right=0) for i in range(3))
+    np.testing.assert_allclose(a[0], ref, rtol=1e-12, atol=1e-12)
+
+
+# ---- P6: a single point absorber peaks at its own pixel (north_star check 2) ---------------
+@pytest.mark.parametrize("mode,pulse", [(0, "gaussian"), (1, "bipolar")])
+def test_p6_point_source_peaks_at_its_pixel(mode, pulse):
+    g = W.make_geometry(0)
+    tau = oracle.fmm_rows(g.n, g.h, g.origin, g.c_map, g.sensors.astype(np.float64), g.roi_index)
+    xy = g.roi_coords()
+    for node in (32 * 64 + 32, 25 * 64 + 40, 38 * 64 + 22, 20 * 64 + 30):
+        assert np.hypot(*xy[node]) < 10e-3
+        tr = W.make_traces(g, tau, frames=[0], noise_sigma=0.0, pulse=pulse,
+                           absorbers=[(np.array([node]), np.array([1.0]))])
+        img = oracle.backproject(tau, tr, g.fs, mode=mode)[0]
+        assert int(np.argmax(img)) == node
+
+
+def test_pitch_and_empty_inputs():
+    rng = np.random.default_rng(11)
+    tau, tr = _rand_case(rng, S=3, P=20, Nt=32, B=1)
+    wide = np.zeros((3, 32), np.float32)
+    wide[:, :20] = tau
+    np.testing.assert_array_equal(oracle.backproject(wide[:, :20], tr, FS), oracle.backproject(tau, tr, FS))
+    assert oracle.backproject(tau[:, :0], tr, FS).shape == (1, 0)
