@@ -1,0 +1,147 @@
+/*
+ * pat.h -- C-ABI of the B200-native phase-corrected back projection
+ * (Wang & Jing, arxiv 1501.03869; hot path = Eq. 7).
+ *
+ * One GPU (sm_100a), fp32, no CPU fallback: on a machine without a usable
+ * sm_100 device every call that needs the device returns PAT_ERR_UNSUPPORTED
+ * or PAT_ERR_CUDA -- nothing is ever computed on the host in its place.
+ *
+ * Conventions
+ *   - every entry point returns a pat_status; nothing throws, aborts or prints;
+ *   - *out is written only on PAT_OK;
+ *   - all arrays are caller-owned and only BORROWED: host arrays until the call
+ *     returns, the device workspace until pat_destroy, traces/images until the
+ *     work enqueued on `stream` has completed;
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream);
+ *   - a plan is not thread-safe; different plans may be used concurrently;
+ *   - grids are node-centred, x fastest: linear index = ix + n[0]*(iy + n[1]*iz),
+ *     node coordinates = origin + index*h.
+ */
+#ifndef PAT_H_
+#define PAT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pat_plan pat_plan;               /* opaque, host-side */
+
+typedef enum {
+    PAT_OK = 0,
+    PAT_ERR_INVALID_ARG = 1,
+    PAT_ERR_BAD_STATE = 2,      /* e.g. pat_backproject before every sensor row was set */
+    PAT_ERR_CUDA = 3,           /* CUDA runtime failure; text in pat_last_error */
+    PAT_ERR_NOMEM = 4,          /* host allocation failed or workspace too small */
+    PAT_ERR_UNSUPPORTED = 5     /* device is not sm_100 (no fallback path exists) */
+} pat_status;
+
+/* BP weighting b = wp*p - wd*t*dp/dt applied to the traces (reading R1). */
+typedef enum {
+    PAT_W_DELAY_SUM = 0,        /* p                         (plain delay-and-sum)          */
+    PAT_W_PAPER = 1,            /* p - t*dp/dt               (Eq. 7 as printed) */
+    PAT_W_UBP = 2               /* 2p - 2t*dp/dt             (universal BP, ref. [5])        */
+} pat_weighting;
+
+/* Regular grid of the speed-of-sound map / FMM domain. */
+typedef struct {
+    int32_t ndim;               /* 2 or 3 */
+    int32_t n[3];               /* nodes per axis, x fastest; n[2] = 1 in 2-D */
+    float   h;                  /* isotropic spacing [m] (paper: 0.195e-3 / 0.39e-3) */
+    float   origin[3];          /* coordinates of node (0,0,0) [m] */
+} pat_grid;
+
+/* Bytes of DEVICE workspace a plan with these sizes needs (0 on invalid sizes).
+ * Layout: re-tiled tau table (the dominant term, 4*nsens*npix rounded up to whole
+ * 256-pixel tiles), weighted traces for max_batch frames, staging for host-side
+ * inputs, pixel permutation. */
+size_t pat_plan_workspace_bytes(const pat_grid *grid, int32_t nsens, int64_t npix,
+                                int32_t nt, int32_t max_batch);
+
+/* pat_plan_create -- the paper's problem statement.
+ *   grid        FMM / c-map grid.
+ *   c_map       HOST fp32 [n0*n1*n2] speed of sound [m/s]; copied into the plan for
+ *               pat_compute_travel_times; may be NULL if the caller supplies tau itself.
+ *               Every entry must be finite and > 0.
+ *   sensor_xyz  HOST fp32 [nsens*3] sensor positions [m]; copied; may be NULL (as c_map).
+ *   roi_index   HOST int64 [npix] strictly ascending linear node indices of the pixels to
+ *               reconstruct ("the area within the skull"); NULL => all nodes
+ *               (npix must then equal n0*n1*n2).
+ *   nt, fs, t0  trace sampling: sample n is at time t0 + n/fs; nt >= 2, fs > 0.
+ *   weighting   pat_weighting.
+ *   max_batch   largest nframes a pat_backproject call will pass (>= 1).
+ *   workspace   DEVICE memory, 256-byte aligned, >= pat_plan_workspace_bytes(...), owned by
+ *               the caller (e.g. a torch tensor) and borrowed until pat_destroy.
+ * Errors: NULL out/grid/workspace, bad sizes, non-ascending or out-of-grid roi_index,
+ * bad c_map entry, misaligned or too small workspace -> PAT_ERR_INVALID_ARG (argument checks
+ * run before any CUDA call); no sm_100 device -> PAT_ERR_UNSUPPORTED; CUDA failure -> PAT_ERR_CUDA. */
+pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, const float *c_map,
+                           const float *sensor_xyz, int32_t nsens,
+                           const int64_t *roi_index, int64_t npix,
+                           int32_t nt, float fs, float t0,
+                           int32_t weighting, int32_t max_batch,
+                           void *workspace, size_t workspace_bytes);
+
+/* pat_set_travel_times -- hand the plan rows of the tau table.
+ *   tau   fp32 seconds, row-major [count][npix] (pixel order = roi_index order) for sensors
+ *         [sensor_begin, sensor_begin+count).  HOST or DEVICE pointer (detected).
+ * Copies and re-tiles the rows into the workspace (spatially compact 256-pixel tiles) on
+ * `stream`; a host source is staged in pieces, so the call returns after the host buffer has
+ * been consumed.  May be called repeatedly with disjoint sensor ranges (the 34 GB 3-D table).
+ * Values that are negative, NaN, +-inf or beyond the record are LEGAL and contribute 0. */
+pat_status pat_set_travel_times(pat_plan *plan, const float *tau, int32_t sensor_begin,
+                                int32_t count, void *stream);
+
+/* pat_backproject -- Eq. 7 for nframes frames:
+ *     images[f][j] = sum_i (1-a)*b_fi[k] + a*b_fi[k+1],   u = fl32(fl32(tau_ij - t0)*fs),
+ *     k = floor(u), a = u - k, terms with !(0 <= u < nt-1) contribute 0,
+ *     b_fi[n] = wp*p_fi[n] - wd*(n + t0*fs)*D_fi[n]   (central differences, one-sided ends).
+ *   traces  fp32 [nframes][nsens][nt]     images  fp32 [nframes][npix] (roi_index order)
+ * Both DEVICE (16-byte aligned) or both HOST pointers (detected; host buffers should be
+ * pinned for the copies to be asynchronous).  Enqueues weighting pre-pass + gather (+ the
+ * copies for host buffers) on `stream` and returns without synchronising.
+ * nframes = 0 is a no-op; nframes > max_batch -> PAT_ERR_INVALID_ARG; tau rows missing ->
+ * PAT_ERR_BAD_STATE. */
+pat_status pat_backproject(pat_plan *plan, const float *traces, float *images,
+                           int32_t nframes, void *stream);
+
+/* Frees the host-side plan; never frees caller memory.  NULL is allowed. */
+pat_status pat_destroy(pat_plan *plan);
+
+/* ---- helpers ------------------------------------------------------------------------ */
+
+/* Last error text of a plan (or of the last failed pat_plan_create when plan == NULL).
+ * Never NULL; owned by the library. */
+const char *pat_last_error(const pat_plan *plan);
+
+/* Number of kernels of this library launched through `plan` so far (monotone counter). */
+int64_t pat_kernel_launches(const pat_plan *plan);
+
+/* Select the gather implementation: 0 = automatic, 1 = pixel-lane (one thread per pixel,
+ * traces gathered through L1), 2 = frame-lane (lanes = frames, trace windows staged in
+ * shared memory).  PAT_ERR_UNSUPPORTED if the variant cannot run this plan. */
+pat_status pat_set_gather_variant(pat_plan *plan, int32_t variant);
+
+/* pat_fmm_travel_times -- UNTIMED input preparation, HOST only: the
+ * first-order upwind, heap-ordered narrow-band fast marching solve of |grad T| = 1/c from
+ * each sensor (reciprocity); order = 2 uses the paper's Eq. 6 stencil with
+ * first-order fallback.  Rows for sensors [sensor_begin, sensor_begin+count) of sensor_xyz:
+ *   tau_out  HOST fp32 [count][npix], T computed in double and rounded once.
+ *   nthreads OpenMP threads over sensors (<= 0: all cores).
+ * A sensor outside the grid -> PAT_ERR_INVALID_ARG. */
+pat_status pat_fmm_travel_times(const pat_grid *grid, const float *c_map,
+                                const float *sensor_xyz, int32_t nsens,
+                                const int64_t *roi_index, int64_t npix,
+                                int32_t sensor_begin, int32_t count, int32_t order,
+                                float *tau_out, int32_t nthreads);
+
+/* Convenience: run pat_fmm_travel_times on the plan's own grid / c_map / sensors (both must
+ * have been given to pat_plan_create) in chunks and feed every row to pat_set_travel_times. */
+pat_status pat_compute_travel_times(pat_plan *plan, int32_t order, int32_t nthreads, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PAT_H_ */

@@ -1,0 +1,14 @@
+"""B200-native phase-corrected back projection (arxiv 1501.03869, Eq. 7).
+
+The product is the C-ABI library built from csrc/ (libpat_b200.so, sm_100a); this package
+is a thin ctypes binding with the same entry-point names.  There is no CPU fallback: the
+import fails loudly if the library is missing, and every compute call needs a B200.
+"""
+from .binding import (PAT_OK, PAT_ERR_INVALID_ARG, PAT_ERR_BAD_STATE, PAT_ERR_CUDA, PAT_ERR_NOMEM,
+                      PAT_ERR_UNSUPPORTED, PAT_W_DELAY_SUM, PAT_W_PAPER, PAT_W_UBP, PatError, PatGrid,
+                      lib, library_path, pat_plan_workspace_bytes, pat_plan_create,
+                      pat_set_travel_times, pat_backproject, pat_destroy, pat_last_error,
+                      pat_kernel_launches, pat_set_gather_variant, pat_fmm_travel_times,
+                      pat_compute_travel_times, Plan)
+
+__all__ = [n for n in dir() if n.startswith(("pat_", "PAT_", "Pat", "Plan", "lib"))]

@@ -1,0 +1,220 @@
+"""ctypes binding of include/pat.h -- argument marshalling only.
+
+Every function has the name and argument order of its C counterpart.  Arrays may be numpy
+arrays (host) or torch tensors (host or CUDA); a raw integer address is also accepted.
+`Plan` is a small convenience owner of the handle and of the torch workspace tensor.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+PAT_OK, PAT_ERR_INVALID_ARG, PAT_ERR_BAD_STATE, PAT_ERR_CUDA, PAT_ERR_NOMEM, PAT_ERR_UNSUPPORTED = range(6)
+PAT_W_DELAY_SUM, PAT_W_PAPER, PAT_W_UBP = 0, 1, 2
+_STATUS = ["PAT_OK", "PAT_ERR_INVALID_ARG", "PAT_ERR_BAD_STATE", "PAT_ERR_CUDA", "PAT_ERR_NOMEM",
+           "PAT_ERR_UNSUPPORTED"]
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBNAME = "libpat_b200.so"
+
+
+class PatError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__("%s: %s" % (_STATUS[status] if 0 <= status < len(_STATUS) else status, msg))
+        self.status = status
+
+
+class PatGrid(ctypes.Structure):
+    _fields_ = [("ndim", ctypes.c_int32), ("n", ctypes.c_int32 * 3), ("h", ctypes.c_float),
+                ("origin", ctypes.c_float * 3)]
+
+    @classmethod
+    def make(cls, n, h, origin):
+        g = cls()
+        g.ndim = len(n)
+        for d in range(3):
+            g.n[d] = int(n[d]) if d < len(n) else 1
+            g.origin[d] = float(origin[d]) if d < len(origin) else 0.0
+        g.h = float(h)
+        return g
+
+
+def library_path():
+    return os.path.join(_HERE, _LIBNAME)
+
+
+_lib = None
+
+
+def lib():
+    """Load libpat_b200.so (built in-tree by paper_1501_03869_b200/build.py). No fallback."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = library_path()
+    if not os.path.exists(path):
+        raise ImportError(
+            "%s is missing: build it with `python -m paper_1501_03869_b200.build` "
+            "(nvcc, sm_100a). There is no CPU or PyTorch fallback for this package." % path)
+    L = ctypes.CDLL(path)
+    i32, i64, f32, vp, sz = ctypes.c_int32, ctypes.c_int64, ctypes.c_float, ctypes.c_void_p, ctypes.c_size_t
+    gp = ctypes.POINTER(PatGrid)
+    L.pat_plan_workspace_bytes.restype = sz
+    L.pat_plan_workspace_bytes.argtypes = [gp, i32, i64, i32, i32]
+    L.pat_plan_create.restype = ctypes.c_int
+    L.pat_plan_create.argtypes = [ctypes.POINTER(vp), gp, vp, vp, i32, vp, i64, i32, f32, f32, i32, i32, vp, sz]
+    L.pat_set_travel_times.restype = ctypes.c_int
+    L.pat_set_travel_times.argtypes = [vp, vp, i32, i32, vp]
+    L.pat_backproject.restype = ctypes.c_int
+    L.pat_backproject.argtypes = [vp, vp, vp, i32, vp]
+    L.pat_destroy.restype = ctypes.c_int
+    L.pat_destroy.argtypes = [vp]
+    L.pat_last_error.restype = ctypes.c_char_p
+    L.pat_last_error.argtypes = [vp]
+    L.pat_kernel_launches.restype = i64
+    L.pat_kernel_launches.argtypes = [vp]
+    L.pat_set_gather_variant.restype = ctypes.c_int
+    L.pat_set_gather_variant.argtypes = [vp, i32]
+    L.pat_fmm_travel_times.restype = ctypes.c_int
+    L.pat_fmm_travel_times.argtypes = [gp, vp, vp, i32, vp, i64, i32, i32, i32, vp, i32]
+    L.pat_compute_travel_times.restype = ctypes.c_int
+    L.pat_compute_travel_times.argtypes = [vp, i32, i32, vp]
+    _lib = L
+    return L
+
+
+def _addr(a):
+    """Address of a numpy array, a torch tensor, an int, or None."""
+    if a is None:
+        return None
+    if isinstance(a, int):
+        return a
+    if isinstance(a, np.ndarray):
+        if not a.flags["C_CONTIGUOUS"]:
+            raise ValueError("array must be C-contiguous")
+        return a.ctypes.data
+    if hasattr(a, "data_ptr"):
+        if not a.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        return a.data_ptr()
+    raise TypeError("expected numpy array, torch tensor, int address or None")
+
+
+def _stream(stream):
+    if stream is None:
+        return None
+    if isinstance(stream, int):
+        return stream or None
+    return stream.cuda_stream or None            # torch.cuda.Stream
+
+
+def _check(plan, st):
+    if st != PAT_OK:
+        raise PatError(st, pat_last_error(plan))
+    return st
+
+
+def pat_plan_workspace_bytes(grid, nsens, npix, nt, max_batch):
+    return int(lib().pat_plan_workspace_bytes(ctypes.byref(grid), nsens, npix, nt, max_batch))
+
+
+def pat_plan_create(grid, c_map, sensor_xyz, nsens, roi_index, npix, nt, fs, t0, weighting, max_batch,
+                    workspace, workspace_bytes):
+    """Returns the opaque plan handle (int). Raises PatError on failure."""
+    for arr, dt in ((c_map, np.float32), (sensor_xyz, np.float32), (roi_index, np.int64)):
+        if isinstance(arr, np.ndarray) and arr.dtype != dt:
+            raise TypeError("host array has dtype %s, expected %s" % (arr.dtype, np.dtype(dt)))
+    h = ctypes.c_void_p()
+    st = lib().pat_plan_create(ctypes.byref(h), ctypes.byref(grid), _addr(c_map), _addr(sensor_xyz), nsens,
+                               _addr(roi_index), npix, nt, fs, t0, weighting, max_batch,
+                               _addr(workspace), workspace_bytes)
+    _check(None, st)
+    return h.value
+
+
+def pat_set_travel_times(plan, tau, sensor_begin, count, stream=None):
+    if isinstance(tau, np.ndarray) and tau.dtype != np.float32:
+        raise TypeError("tau must be float32")
+    return _check(plan, lib().pat_set_travel_times(plan, _addr(tau), sensor_begin, count, _stream(stream)))
+
+
+def pat_backproject(plan, traces, images, nframes, stream=None):
+    return _check(plan, lib().pat_backproject(plan, _addr(traces), _addr(images), nframes, _stream(stream)))
+
+
+def pat_destroy(plan):
+    return lib().pat_destroy(plan)
+
+
+def pat_last_error(plan):
+    return lib().pat_last_error(plan).decode()
+
+
+def pat_kernel_launches(plan):
+    return int(lib().pat_kernel_launches(plan))
+
+
+def pat_set_gather_variant(plan, variant):
+    return _check(plan, lib().pat_set_gather_variant(plan, variant))
+
+
+def pat_fmm_travel_times(grid, c_map, sensor_xyz, nsens, roi_index, npix, sensor_begin, count, order,
+                         tau_out, nthreads=0):
+    st = lib().pat_fmm_travel_times(ctypes.byref(grid), _addr(c_map), _addr(sensor_xyz), nsens,
+                                    _addr(roi_index), npix, sensor_begin, count, order, _addr(tau_out), nthreads)
+    if st != PAT_OK:
+        raise PatError(st, "pat_fmm_travel_times")
+    return st
+
+
+def pat_compute_travel_times(plan, order=1, nthreads=0, stream=None):
+    return _check(plan, lib().pat_compute_travel_times(plan, order, nthreads, _stream(stream)))
+
+
+class Plan:
+    """Owns a plan handle and its torch workspace tensor (device memory stays torch's)."""
+
+    def __init__(self, n, h, origin, c_map, sensor_xyz, roi_index, nt, fs, t0=0.0,
+                 weighting=PAT_W_PAPER, max_batch=1, device="cuda"):
+        import torch
+        self.grid = PatGrid.make(n, h, origin)
+        self.c_map = None if c_map is None else np.ascontiguousarray(c_map, dtype=np.float32).ravel()
+        self.sensor_xyz = None if sensor_xyz is None else np.ascontiguousarray(sensor_xyz, dtype=np.float32)
+        self.roi_index = None if roi_index is None else np.ascontiguousarray(roi_index, dtype=np.int64)
+        self.nsens = int(self.sensor_xyz.shape[0]) if self.sensor_xyz is not None else None
+        self.npix = int(self.roi_index.size) if self.roi_index is not None else int(np.prod(n))
+        self.nt, self.fs, self.t0, self.max_batch = int(nt), float(fs), float(t0), int(max_batch)
+        nbytes = pat_plan_workspace_bytes(self.grid, self.nsens, self.npix, self.nt, self.max_batch)
+        if nbytes == 0:
+            raise PatError(PAT_ERR_INVALID_ARG, "invalid plan sizes")
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=device)
+        base = self.workspace.data_ptr()
+        self._ws_addr = (base + 255) // 256 * 256
+        self.handle = pat_plan_create(self.grid, self.c_map, self.sensor_xyz, self.nsens, self.roi_index,
+                                      self.npix, self.nt, self.fs, self.t0, weighting, self.max_batch,
+                                      self._ws_addr, nbytes)
+
+    def set_travel_times(self, tau, sensor_begin=0, count=None, stream=None):
+        count = int(tau.shape[0]) if count is None else count
+        return pat_set_travel_times(self.handle, tau, sensor_begin, count, stream)
+
+    def compute_travel_times(self, order=1, nthreads=0, stream=None):
+        return pat_compute_travel_times(self.handle, order, nthreads, stream)
+
+    def backproject(self, traces, images, nframes=None, stream=None):
+        nframes = int(traces.shape[0]) if nframes is None else nframes
+        return pat_backproject(self.handle, traces, images, nframes, stream)
+
+    def launches(self):
+        return pat_kernel_launches(self.handle)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            pat_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,325 @@
+// pat_api.cu -- the C-ABI of include/pat.h: argument checking, workspace layout, plan state,
+// stream-ordered orchestration of the kernels.  No arithmetic of the method runs on the host.
+#include "pat_internal.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <numeric>
+
+namespace {
+
+std::string g_create_error;            // last pat_plan_create failure (plan == NULL in pat_last_error)
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+pat_status fail(pat_plan *p, pat_status st, const std::string &msg) {
+    if (p) p->err = msg; else g_create_error = msg;
+    return st;
+}
+pat_status cuda_fail(pat_plan *p, int e, const char *what) {
+    std::string m = std::string(what) + ": " + cudaGetErrorString((cudaError_t)e);
+    cudaGetLastError();                // clear the sticky-less error state
+    return fail(p, PAT_ERR_CUDA, m);
+}
+
+bool dims_ok(const pat_grid *g, int32_t nsens, int64_t npix, int32_t nt, int32_t max_batch) {
+    if (!g || (g->ndim != 2 && g->ndim != 3)) return false;
+    int64_t N = 1;
+    for (int d = 0; d < g->ndim; ++d) {
+        if (g->n[d] < 2) return false;
+        N *= g->n[d];
+        if (N > (int64_t)INT32_MAX) return false;
+    }
+    if (!(g->h > 0.0f) || !std::isfinite(g->h)) return false;
+    if (nsens <= 0 || npix <= 0 || npix > N || nt < 2 || max_batch < 1) return false;
+    if ((int64_t)nt > (1 << 22)) return false;              // k is recovered from a 2^23-biased float
+    return true;
+}
+
+// Is `p` device memory?  1 = device/managed, 0 = host (pinned or pageable), -1 = query failed.
+int is_device_ptr(const void *p) {
+    cudaPointerAttributes a{};
+    cudaError_t e = cudaPointerGetAttributes(&a, p);
+    if (e != cudaSuccess) { cudaGetLastError(); return -1; }
+    return (a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged) ? 1 : 0;
+}
+
+// 64-bit Morton key of a node (x fastest); keeps 256 consecutive ROI pixels spatially compact.
+inline uint64_t spread2(uint32_t v) {
+    uint64_t x = v;
+    x = (x | (x << 16)) & 0x0000FFFF0000FFFFull;
+    x = (x | (x << 8)) & 0x00FF00FF00FF00FFull;
+    x = (x | (x << 4)) & 0x0F0F0F0F0F0F0F0Full;
+    x = (x | (x << 2)) & 0x3333333333333333ull;
+    x = (x | (x << 1)) & 0x5555555555555555ull;
+    return x;
+}
+inline uint64_t spread3(uint32_t v) {
+    uint64_t x = v & 0x1FFFFF;
+    x = (x | (x << 32)) & 0x1F00000000FFFFull;
+    x = (x | (x << 16)) & 0x1F0000FF0000FFull;
+    x = (x | (x << 8)) & 0x100F00F00F00F00Full;
+    x = (x | (x << 4)) & 0x10C30C30C30C30C3ull;
+    x = (x | (x << 2)) & 0x1249249249249249ull;
+    return x;
+}
+
+}  // namespace
+
+PatLayout pat_layout(const PatDims &d) {
+    PatLayout L;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+    L.tau = take((size_t)d.ntiles * d.nsens * kTilePix * sizeof(float));
+    L.bd = take((size_t)d.max_batch * d.nsens * d.nt * 2 * sizeof(float));
+    L.perm = take((size_t)d.ntiles * kTilePix * sizeof(int32_t));
+    L.traces = take((size_t)d.max_batch * d.nsens * d.nt * sizeof(float));
+    L.images = take((size_t)d.max_batch * d.npix * sizeof(float));
+    int64_t rows = (int64_t)((32u << 20) / ((size_t)d.npix * sizeof(float)));
+    rows = std::max<int64_t>(1, std::min<int64_t>(rows, d.nsens));
+    L.stage_rows = rows;
+    L.tau_stage = take((size_t)rows * d.npix * sizeof(float));
+    L.total = off;
+    return L;
+}
+
+extern "C" size_t pat_plan_workspace_bytes(const pat_grid *grid, int32_t nsens, int64_t npix,
+                                           int32_t nt, int32_t max_batch) {
+    if (!dims_ok(grid, nsens, npix, nt, max_batch)) return 0;
+    PatDims d;
+    d.nsens = nsens; d.npix = npix; d.nt = nt; d.max_batch = max_batch;
+    d.ntiles = (npix + kTilePix - 1) / kTilePix;
+    return pat_layout(d).total;
+}
+
+extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, const float *c_map,
+                                      const float *sensor_xyz, int32_t nsens,
+                                      const int64_t *roi_index, int64_t npix,
+                                      int32_t nt, float fs, float t0,
+                                      int32_t weighting, int32_t max_batch,
+                                      void *workspace, size_t workspace_bytes) {
+    // ---- argument checks: all of them run before the first CUDA call ---------------------
+    if (!out) return fail(nullptr, PAT_ERR_INVALID_ARG, "out is NULL");
+    if (!grid) return fail(nullptr, PAT_ERR_INVALID_ARG, "grid is NULL");
+    if (!dims_ok(grid, nsens, npix, nt, max_batch))
+        return fail(nullptr, PAT_ERR_INVALID_ARG, "bad sizes (ndim, n, h, nsens, npix, nt or max_batch)");
+    if (!(fs > 0.0f) || !std::isfinite(fs) || !std::isfinite(t0))
+        return fail(nullptr, PAT_ERR_INVALID_ARG, "fs must be finite and > 0, t0 finite");
+    if (weighting < 0 || weighting > 2) return fail(nullptr, PAT_ERR_INVALID_ARG, "unknown weighting");
+    int64_t N = 1;
+    for (int d = 0; d < grid->ndim; ++d) N *= grid->n[d];
+    if (!roi_index && npix != N)
+        return fail(nullptr, PAT_ERR_INVALID_ARG, "roi_index NULL requires npix == number of nodes");
+    if (roi_index)
+        for (int64_t j = 0; j < npix; ++j) {
+            if (roi_index[j] < 0 || roi_index[j] >= N || (j > 0 && roi_index[j] <= roi_index[j - 1]))
+                return fail(nullptr, PAT_ERR_INVALID_ARG, "roi_index must be strictly ascending and inside the grid");
+        }
+    if (c_map)
+        for (int64_t q = 0; q < N; ++q)
+            if (!(c_map[q] > 0.0f) || !std::isfinite(c_map[q]))
+                return fail(nullptr, PAT_ERR_INVALID_ARG, "c_map entries must be finite and > 0");
+    if (sensor_xyz)
+        for (int64_t q = 0; q < (int64_t)nsens * 3; ++q)
+            if (!std::isfinite(sensor_xyz[q]))
+                return fail(nullptr, PAT_ERR_INVALID_ARG, "sensor_xyz must be finite");
+    if (!workspace) return fail(nullptr, PAT_ERR_INVALID_ARG, "workspace is NULL");
+    if (((uintptr_t)workspace & 255u) != 0)
+        return fail(nullptr, PAT_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+
+    pat_plan *p = new (std::nothrow) pat_plan();
+    if (!p) return fail(nullptr, PAT_ERR_NOMEM, "host allocation failed");
+    p->dims.nsens = nsens; p->dims.npix = npix; p->dims.nt = nt; p->dims.max_batch = max_batch;
+    p->dims.ntiles = (npix + kTilePix - 1) / kTilePix;
+    p->lay = pat_layout(p->dims);
+    if (workspace_bytes < p->lay.total) {
+        delete p;
+        return fail(nullptr, PAT_ERR_INVALID_ARG, "workspace smaller than pat_plan_workspace_bytes");
+    }
+    p->grid = *grid;
+    if (grid->ndim == 2) { p->grid.n[2] = 1; p->grid.origin[2] = 0.0f; }
+    p->fs = fs; p->t0 = t0; p->weighting = weighting;
+    p->wp = weighting == PAT_W_UBP ? 2.0f : 1.0f;
+    p->wd = weighting == PAT_W_DELAY_SUM ? 0.0f : p->wp;
+    p->ws = (char *)workspace;
+    const char *env = std::getenv("PAT_NO_PDL");
+    p->use_pdl = !(env && env[0] == '1');
+
+    std::vector<int32_t> perm;
+    try {
+        p->row_set.assign((size_t)nsens, 0);
+        if (c_map) p->c_map.assign(c_map, c_map + N);
+        if (sensor_xyz) p->sensors.assign(sensor_xyz, sensor_xyz + (int64_t)nsens * 3);
+        if (roi_index) p->roi.assign(roi_index, roi_index + npix);
+        // spatially compact pixel order: sort ROI positions by the Morton key of their node
+        std::vector<uint64_t> key((size_t)npix);
+        const int64_t n0 = grid->n[0], n1 = grid->n[1];
+        for (int64_t j = 0; j < npix; ++j) {
+            const int64_t q = roi_index ? roi_index[j] : j;
+            const uint32_t ix = (uint32_t)(q % n0), iy = (uint32_t)((q / n0) % n1), iz = (uint32_t)(q / (n0 * n1));
+            key[j] = grid->ndim == 2 ? (spread2(ix) | (spread2(iy) << 1))
+                                     : (spread3(ix) | (spread3(iy) << 1) | (spread3(iz) << 2));
+        }
+        perm.assign((size_t)p->dims.ntiles * kTilePix, -1);
+        std::iota(perm.begin(), perm.begin() + npix, 0);
+        std::sort(perm.begin(), perm.begin() + npix,
+                  [&](int32_t a, int32_t b) { return key[a] < key[b] || (key[a] == key[b] && a < b); });
+    } catch (...) {
+        delete p;
+        return fail(nullptr, PAT_ERR_NOMEM, "host allocation failed");
+    }
+
+    // ---- device ---------------------------------------------------------------------------
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { delete p; return cuda_fail(nullptr, e, "cudaGetDevice (no usable CUDA device; there is no CPU fallback)"); }
+    int major = 0, sms = 0;
+    e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) { delete p; return cuda_fail(nullptr, e, "cudaDeviceGetAttribute"); }
+    if (major != 10) {
+        delete p;
+        return fail(nullptr, PAT_ERR_UNSUPPORTED, "device is not sm_100 (Blackwell B200); no fallback path exists");
+    }
+    if (is_device_ptr(workspace) != 1) {
+        delete p;
+        return fail(nullptr, PAT_ERR_INVALID_ARG, "workspace is not device memory");
+    }
+    p->device = dev;
+    p->num_sms = sms;
+    e = cudaMemcpy(p->ws + p->lay.perm, perm.data(), perm.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { delete p; return cuda_fail(nullptr, e, "upload of the pixel permutation"); }
+    *out = p;
+    return PAT_OK;
+}
+
+extern "C" pat_status pat_set_travel_times(pat_plan *p, const float *tau, int32_t sensor_begin,
+                                           int32_t count, void *stream) {
+    if (!p) return PAT_ERR_INVALID_ARG;
+    if (!tau && count > 0) return fail(p, PAT_ERR_INVALID_ARG, "tau is NULL");
+    if (sensor_begin < 0 || count < 0 || sensor_begin > p->dims.nsens - count)
+        return fail(p, PAT_ERR_INVALID_ARG, "sensor range outside [0, nsens)");
+    if (count == 0) return PAT_OK;
+    const int on_dev = is_device_ptr(tau);
+    if (on_dev < 0) return fail(p, PAT_ERR_CUDA, "cudaPointerGetAttributes failed on tau");
+    cudaStream_t st = (cudaStream_t)stream;
+    PatLaunchCtx ctx{stream, p->num_sms, p->use_pdl};
+    float *tau_t = (float *)(p->ws + p->lay.tau);
+    const int32_t *perm = (const int32_t *)(p->ws + p->lay.perm);
+    const int64_t P = p->dims.npix;
+    if (on_dev) {
+        int e = pat_launch_retile(ctx, tau, tau_t, perm, p->dims.nsens, P, p->dims.ntiles, sensor_begin, count);
+        if (e) return cuda_fail(p, e, "retile launch");
+        ++p->launches;
+    } else {
+        float *stage = (float *)(p->ws + p->lay.tau_stage);
+        for (int32_t r = 0; r < count; r += (int32_t)p->lay.stage_rows) {
+            const int32_t m = (int32_t)std::min<int64_t>(p->lay.stage_rows, count - r);
+            cudaError_t e = cudaMemcpyAsync(stage, tau + (int64_t)r * P, (size_t)m * P * sizeof(float),
+                                            cudaMemcpyHostToDevice, st);
+            if (e != cudaSuccess) return cuda_fail(p, e, "tau H2D copy");
+            int le = pat_launch_retile(ctx, stage, tau_t, perm, p->dims.nsens, P, p->dims.ntiles,
+                                       sensor_begin + r, m);
+            if (le) return cuda_fail(p, le, "retile launch");
+            ++p->launches;
+            // the staging buffer is reused by the next piece and the host rows are only
+            // borrowed until return: wait for this piece.
+            e = cudaStreamSynchronize(st);
+            if (e != cudaSuccess) return cuda_fail(p, e, "tau staging synchronise");
+        }
+    }
+    for (int32_t s = sensor_begin; s < sensor_begin + count; ++s)
+        if (!p->row_set[s]) { p->row_set[s] = 1; ++p->rows_set; }
+    return PAT_OK;
+}
+
+extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *images,
+                                      int32_t nframes, void *stream) {
+    if (!p) return PAT_ERR_INVALID_ARG;
+    if (nframes < 0 || nframes > p->dims.max_batch)
+        return fail(p, PAT_ERR_INVALID_ARG, "nframes outside [0, max_batch]");
+    if (nframes == 0) return PAT_OK;
+    if (!traces || !images) return fail(p, PAT_ERR_INVALID_ARG, "traces or images is NULL");
+    if (p->rows_set != p->dims.nsens)
+        return fail(p, PAT_ERR_BAD_STATE, "pat_backproject before every tau row was set");
+    const int td = is_device_ptr(traces), id = is_device_ptr(images);
+    if (td < 0 || id < 0) return fail(p, PAT_ERR_CUDA, "cudaPointerGetAttributes failed");
+    if (td != id) return fail(p, PAT_ERR_INVALID_ARG, "traces and images must both be host or both device");
+    if (td && ((((uintptr_t)traces) | ((uintptr_t)images)) & 15u))
+        return fail(p, PAT_ERR_INVALID_ARG, "device traces/images must be 16-byte aligned");
+
+    cudaStream_t st = (cudaStream_t)stream;
+    const PatDims &d = p->dims;
+    const float *d_tr = traces;
+    float *d_img = images;
+    if (!td) {
+        d_tr = (const float *)(p->ws + p->lay.traces);
+        d_img = (float *)(p->ws + p->lay.images);
+        cudaError_t e = cudaMemcpyAsync((void *)d_tr, traces, (size_t)nframes * d.nsens * d.nt * sizeof(float),
+                                        cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return cuda_fail(p, e, "traces H2D copy");
+    }
+    PatLaunchCtx ctx{stream, p->num_sms, p->use_pdl};
+    float *bd = (float *)(p->ws + p->lay.bd);
+    const float t0fs = (float)((double)p->t0 * (double)p->fs);
+    int e = pat_launch_prepass(ctx, d_tr, bd, d_img, d.nsens, d.nt, nframes, d.npix, p->wp, p->wd, t0fs);
+    if (e) return cuda_fail(p, e, "pre-pass launch");
+    ++p->launches;
+    if (p->variant == 2) return fail(p, PAT_ERR_UNSUPPORTED, "frame-lane gather not available for this plan");
+    e = pat_launch_gather_pixel(ctx, (const float *)(p->ws + p->lay.tau), bd,
+                                (const int32_t *)(p->ws + p->lay.perm), d_img, d.nsens, d.npix, d.ntiles,
+                                d.nt, nframes, p->fs, p->t0);
+    if (e) return cuda_fail(p, e, "gather launch");
+    ++p->launches;
+    if (!td) {
+        cudaError_t ce = cudaMemcpyAsync(images, d_img, (size_t)nframes * d.npix * sizeof(float),
+                                         cudaMemcpyDeviceToHost, st);
+        if (ce != cudaSuccess) return cuda_fail(p, ce, "images D2H copy");
+    }
+    return PAT_OK;
+}
+
+extern "C" pat_status pat_destroy(pat_plan *p) {
+    delete p;
+    return PAT_OK;
+}
+
+extern "C" const char *pat_last_error(const pat_plan *p) {
+    return p ? p->err.c_str() : g_create_error.c_str();
+}
+
+extern "C" int64_t pat_kernel_launches(const pat_plan *p) { return p ? p->launches : 0; }
+
+extern "C" pat_status pat_set_gather_variant(pat_plan *p, int32_t variant) {
+    if (!p) return PAT_ERR_INVALID_ARG;
+    if (variant < 0 || variant > 2) return fail(p, PAT_ERR_INVALID_ARG, "variant must be 0, 1 or 2");
+    if (variant == 2) return fail(p, PAT_ERR_UNSUPPORTED, "frame-lane gather not available for this plan");
+    p->variant = variant;
+    return PAT_OK;
+}
+
+extern "C" pat_status pat_compute_travel_times(pat_plan *p, int32_t order, int32_t nthreads, void *stream) {
+    if (!p) return PAT_ERR_INVALID_ARG;
+    if (p->c_map.empty() || p->sensors.empty())
+        return fail(p, PAT_ERR_BAD_STATE, "plan was created without c_map / sensor_xyz");
+    const int64_t P = p->dims.npix;
+    int64_t rows = std::max<int64_t>(1, std::min<int64_t>(p->dims.nsens, (int64_t)(256u << 20) / (P * 4)));
+    std::vector<float> buf;
+    try { buf.resize((size_t)rows * P); } catch (...) { return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
+    for (int32_t s = 0; s < p->dims.nsens; s += (int32_t)rows) {
+        const int32_t m = (int32_t)std::min<int64_t>(rows, p->dims.nsens - s);
+        pat_status st = pat_fmm_travel_times(&p->grid, p->c_map.data(), p->sensors.data(), p->dims.nsens,
+                                             p->roi.empty() ? nullptr : p->roi.data(), P, s, m, order,
+                                             buf.data(), nthreads);
+        if (st != PAT_OK) return fail(p, st, "pat_fmm_travel_times failed (sensor outside the grid?)");
+        st = pat_set_travel_times(p, buf.data(), s, m, stream);
+        if (st != PAT_OK) return st;
+    }
+    return PAT_OK;
+}

@@ -192,14 +192,19 @@ def _geom_vol(reduced):
 def make_geometry(k: int, reduced: bool = False) -> Geometry:
     """Geometry of BASELINE.json configs[k]; `reduced` gives the small variants of k = 3, 4."""
     if k == 0:
-        return _geom_tiny()
-    if k in (1, 2):
-        return _geom_paper(k)
-    if k == 3:
-        return _geom_large(reduced)
-    if k == 4:
-        return _geom_vol(reduced)
-    raise ValueError("config index must be 0..4")
+        g = _geom_tiny()
+    elif k in (1, 2):
+        g = _geom_paper(k)
+    elif k == 3:
+        g = _geom_large(reduced)
+    elif k == 4:
+        g = _geom_vol(reduced)
+    else:
+        raise ValueError("config index must be 0..4")
+    # the C-ABI carries h and origin as fp32: hand every consumer the same (rounded) numbers
+    g.h = float(np.float32(g.h))
+    g.origin = tuple(float(np.float32(v)) for v in g.origin)
+    return g
 
 
 def _roi_lookup(geom):
