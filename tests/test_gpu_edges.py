@@ -1,0 +1,139 @@
+"""GPU edge cases of the C-ABI path: ragged sizes, out-of-record / non-finite tau, t0,
+chunked tau upload, device tau, linearity, error paths that need a device."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as W
+from _cases import assert_parity, gpu_backproject
+
+pytestmark = pytest.mark.gpu
+FS = 20e6
+
+
+def _geom(npix, nsens, nt, nx=64, ny=64):
+    """A bare geometry carrying only sizes (tau is supplied directly)."""
+    g = W.make_geometry(0)
+    g.n = (nx, ny)
+    g.c_map = np.full((ny, nx), 1540.0, np.float32)
+    rng = np.random.default_rng(npix + nsens)
+    g.roi_index = np.sort(rng.choice(nx * ny, size=npix, replace=False)).astype(np.int64)
+    g.sensors = np.zeros((nsens, 3), np.float32)
+    g.nt = nt
+    return g
+
+
+@pytest.mark.parametrize("npix,nsens,nt,B", [(1, 1, 2, 1), (255, 3, 17, 1), (257, 17, 33, 2),
+                                             (1000, 33, 100, 3), (4096, 16, 64, 5), (777, 50, 512, 7)])
+def test_ragged_sizes_random_tau(npix, nsens, nt, B):
+    g = _geom(npix, nsens, nt)
+    rng = np.random.default_rng(1)
+    tau = (rng.uniform(-2.0, nt + 1.0, size=(nsens, npix)) / FS).astype(np.float32)
+    tr = rng.standard_normal((B, nsens, nt)).astype(np.float32)
+    for mode in (0, 1):
+        ref = oracle.backproject(tau, tr, FS, 0.0, mode)
+        assert_parity(gpu_backproject(g, tau, tr, mode=mode), ref, "ragged mode %d" % mode)
+
+
+def test_nonfinite_and_out_of_record_tau_contribute_zero():
+    g = _geom(600, 8, 64)
+    rng = np.random.default_rng(2)
+    tau = (rng.uniform(0.0, 62.0, size=(8, 600)) / FS).astype(np.float32)
+    bad = np.array([np.inf, -np.inf, np.nan, -1e-9, 63.0 / FS, 1.0, -3.0, 1e30, -1e30, 3e38], np.float32)
+    tau[3, :bad.size] = bad
+    tau[5, 100:100 + bad.size] = bad
+    tau[0, 0] = 0.0
+    tau[1, 1] = np.float32(62.0) / np.float32(FS)
+    tr = rng.standard_normal((2, 8, 64)).astype(np.float32)
+    ref = oracle.backproject(tau, tr, FS, 0.0, 1)
+    got = gpu_backproject(g, tau, tr)
+    assert np.all(np.isfinite(got))
+    assert_parity(got, ref, "bad tau")
+    # a whole row of invalid tau = that sensor removed
+    tau2 = tau.copy()
+    tau2[2, :] = np.nan
+    ref2 = oracle.backproject(np.delete(tau, 2, axis=0), np.delete(tr, 2, axis=1), FS, 0.0, 1)
+    assert_parity(gpu_backproject(g, tau2, tr), ref2, "nan row")
+
+
+def test_index_rule_is_one_fp32_multiply():
+    """tau chosen so that fl32(tau*fs) and the double product fall on different sides of an integer."""
+    g = _geom(512, 4, 2048)
+    rng = np.random.default_rng(3)
+    ks = rng.integers(1, 2040, size=(4, 512)).astype(np.float64)
+    tau = np.nextafter((ks / FS).astype(np.float32), np.float32(0)).astype(np.float32)
+    tau[::2] = np.nextafter(tau[::2], np.float32(1))
+    tr = rng.standard_normal((1, 4, 2048)).astype(np.float32) * 100
+    ref = oracle.backproject(tau, tr, FS, 0.0, 1)
+    assert_parity(gpu_backproject(g, tau, tr), ref, "index rule")
+
+
+def test_t0_offset():
+    g = _geom(300, 5, 128)
+    rng = np.random.default_rng(4)
+    t0 = float(np.float32(1.7e-6))
+    tau = (t0 + rng.uniform(-3.0, 130.0, size=(5, 300)) / FS).astype(np.float32)
+    tr = rng.standard_normal((2, 5, 128)).astype(np.float32)
+    ref = oracle.backproject(tau, tr, FS, t0, 1)
+    assert_parity(gpu_backproject(g, tau, tr, t0=t0), ref, "t0")
+
+
+def test_chunked_and_device_tau_upload_and_state_machine():
+    import torch
+    import paper_1501_03869_b200 as pat
+    g = _geom(900, 12, 96)
+    rng = np.random.default_rng(5)
+    tau = (rng.uniform(0.0, 94.0, size=(12, 900)) / FS).astype(np.float32)
+    tr = rng.standard_normal((1, 12, 96)).astype(np.float32)
+    ref = oracle.backproject(tau, tr, FS, 0.0, 1)
+    plan = pat.Plan(g.n, g.h, g.origin, g.c_map, g.sensors, g.roi_index, g.nt, FS, 0.0, max_batch=2)
+    d_tr = torch.from_numpy(tr).cuda()
+    img = torch.zeros((1, 900), dtype=torch.float32, device="cuda")
+    plan.set_travel_times(tau[0:5], 0)
+    with pytest.raises(pat.PatError) as ei:
+        plan.backproject(d_tr, img, 1)
+    assert ei.value.status == pat.PAT_ERR_BAD_STATE
+    plan.set_travel_times(torch.from_numpy(tau[5:9]).cuda(), 5)       # device rows
+    plan.set_travel_times(np.ascontiguousarray(tau[9:12]), 9)
+    plan.backproject(d_tr, img, 1)
+    torch.cuda.synchronize()
+    assert_parity(img.cpu().numpy(), ref, "chunked upload")
+    n0 = plan.launches()
+    plan.backproject(d_tr, img, 1)                                     # idempotent: no hidden state
+    torch.cuda.synchronize()
+    assert plan.launches() == n0 + 2
+    assert_parity(img.cpu().numpy(), ref, "second call")
+    with pytest.raises(pat.PatError) as ei:
+        plan.backproject(d_tr, img, 3)
+    assert ei.value.status == pat.PAT_ERR_INVALID_ARG
+    assert plan.backproject(d_tr, img, 0) == pat.PAT_OK
+    with pytest.raises(pat.PatError):
+        plan.backproject(d_tr, torch.zeros((1, 900)), 1)               # host/device mix
+    plan.close()
+
+
+def test_linearity_on_gpu():
+    g = _geom(2000, 20, 256)
+    rng = np.random.default_rng(6)
+    tau = (rng.uniform(0.0, 254.0, size=(20, 2000)) / FS).astype(np.float32)
+    x = (np.round(rng.standard_normal((1, 20, 256)) * 256) / 256).astype(np.float32)
+    y = (np.round(rng.standard_normal((1, 20, 256)) * 256) / 256).astype(np.float32)
+    z = (2 * x - 0.5 * y).astype(np.float32)
+    gx, gy, gz = (gpu_backproject(g, tau, v).astype(np.float64) for v in (x, y, z))
+    assert_parity(gz, 2 * gx - 0.5 * gy, "linearity")
+
+
+def test_compute_travel_times_on_plan_matches_host_fmm():
+    import torch
+    import paper_1501_03869_b200 as pat
+    from _cases import prod_tau
+    geom = W.make_geometry(0)
+    tau = prod_tau(geom)
+    tr = W.make_traces(geom, tau)
+    plan = pat.Plan(geom.n, geom.h, geom.origin, geom.c_map, geom.sensors, geom.roi_index, geom.nt, geom.fs)
+    plan.compute_travel_times()
+    img = torch.zeros((1, geom.npix), dtype=torch.float32, device="cuda")
+    plan.backproject(torch.from_numpy(tr).cuda(), img, 1)
+    torch.cuda.synchronize()
+    assert_parity(img.cpu().numpy(), oracle.backproject(tau, tr, geom.fs), "plan-side FMM")
+    plan.close()
