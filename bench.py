@@ -1,0 +1,467 @@
+"""bench.py -- throughput of the hot path (H1 pre-pass + H2-H4 gather) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config k] [--batch B] [--impl reference]
+
+A "step" is one pat_backproject call (weighting pre-pass + gather) over one batch of B frames of
+the synthetic workload configs[k] (default k = 1: 512 sensors x 21323 pixels, Nt = 2048, B = 1,
+the configuration BASELINE.json's metric is quoted on).  The tau table comes from the library's
+CPU FMM (input preparation, untimed).  Prints ONE JSON line (rank 0):
+
+  value        pixel*sensor updates/s (GUpd/s), whole job, inputs resident in HBM, CUDA events
+               around exactly K steps, max over ranks.  The steps are replayed from a CUDA graph
+               that holds one step on each of R rotating plans (R * tau bytes > 3 x L2, so the tau
+               stream cannot be served from L2).
+  roofline     the gather kernel alone: algorithmic bytes per launch (tau + traces + images,
+               north_star's definition) / its mean duration from CUDA events inside the library
+               (pat_set_profiling), against the measured HBM copy peak of MEASURED_PEAKS.json.
+  e2e          the same metric through the C-ABI with pinned HOST traces/images (H2D + D2H timed).
+  cpu_baseline the oracle (oracle/pat_oracle.c) timed on this box's host cores, rank 0, N = 1.
+  sweep        B = 1..64 on the same geometry (N = 1 only): ms/frame, GUpd/s, HBM fraction and the
+               SM-side (shared-memory bandwidth) fraction, because for B >~ 4 the path is not
+               HBM-bound.
+
+--impl reference times the CPU oracle as it stands on the same config / metric (rank 0 only).
+Nothing here reads /root/reference; all inputs are seeded and synthetic (workloads/).
+"""
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as W  # noqa: E402
+
+METRIC = "pixel-sensor updates/s (GUpd/s) at 512 sensors x 21323 px"
+FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
+NOMINAL_HBM_GBS = 8000.0           # north_star's "~8 TB/s"
+SMEM_BYTES_PER_CLK_SM = 128.0      # B300_MICROARCH.md: shared-memory bandwidth per SM
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs[k] geometry (1, 2, 3, 4)")
+    ap.add_argument("--batch", type=int, default=0, help="frames per step (0 = the config's own batch)")
+    ap.add_argument("--reduced", action="store_true", help="reduced variant of config 3 / 4")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--variant", type=int, default=0, help="pat_set_gather_variant (0 = automatic)")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)", float(d.get("sm_max_mhz", 1965.0))
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)", 1965.0
+
+
+def algorithmic_bytes(S, P, Nt, B):
+    """north_star: tau bytes (once per batch) + trace bytes + image bytes."""
+    return 4.0 * S * P + 4.0 * B * S * Nt + 4.0 * B * P
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi-equivalent clock / throttle-reason samples through NVML while the GPU is loaded."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.stop_flag, self.ok = index, [], False, False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.max_mhz = None
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                rs = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h) if hasattr(
+                    nv, "nvmlDeviceGetCurrentClocksEventReasons") else nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                util = nv.nvmlDeviceGetUtilizationRates(self.h).gpu
+                self.samples.append((mhz, rs, util))
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+        }
+        mhz = [s[0] for s in self.samples]
+        top = max(mhz)
+        load = [m for m in mhz if m >= 0.5 * top] or mhz
+        bits = 0
+        for s in self.samples:
+            bits |= int(s[1])
+        reasons = sorted(n for b, n in names.items() if bits & b)
+        return {"sm_mhz": float(np.median(load)), "sm_max_mhz": self.max_mhz, "reasons": reasons,
+                "samples": len(self.samples)}
+
+
+# ---------------------------------------------------------------------------------------------
+# input preparation (untimed)
+# ---------------------------------------------------------------------------------------------
+def prepare_inputs(k, reduced, nframes, frame0=0):
+    """Geometry, tau (library CPU FMM -- north_star: input preparation, not timed), traces."""
+    import paper_1501_03869_b200 as pat
+    geom = W.make_geometry(k, reduced)
+    grid = pat.PatGrid.make(geom.n, geom.h, geom.origin)
+    tau = np.empty((geom.nsens, geom.npix), dtype=np.float32)
+    pat.pat_fmm_travel_times(grid, np.ascontiguousarray(geom.c_map).ravel(), geom.sensors, geom.nsens,
+                             geom.roi_index, geom.npix, 0, geom.nsens, 1, tau, 0)
+    traces = W.make_traces(geom, tau, frames=range(frame0, frame0 + nframes))
+    return geom, tau, traces
+
+
+class Rig:
+    """R rotating plans (own tau copy, traces, images) so that consecutive steps never find their
+    tau table in L2: R * tau bytes > 3 x L2."""
+
+    def __init__(self, geom, tau, traces, B, variant=0, host=False):
+        import torch
+        import paper_1501_03869_b200 as pat
+        self.pat, self.torch, self.geom, self.B = pat, torch, geom, B
+        props = torch.cuda.get_device_properties(torch.cuda.current_device())
+        l2 = getattr(props, "L2_cache_size", 126 << 20) or (126 << 20)
+        step_bytes = algorithmic_bytes(geom.nsens, geom.npix, geom.nt, B)
+        self.R = int(max(2, min(12, math.ceil(3.0 * l2 / step_bytes))))
+        self.l2_bytes = int(l2)
+        self.plans, self.tr, self.img = [], [], []
+        F = traces.shape[0]
+        for r in range(self.R):
+            p = pat.Plan(geom.n, geom.h, geom.origin, None, geom.sensors, geom.roi_index, geom.nt, geom.fs,
+                         geom.t0, weighting=pat.PAT_W_PAPER, max_batch=B)
+            if variant:
+                pat.pat_set_gather_variant(p.handle, variant)
+            p.set_travel_times(tau)
+            sel = [(r * B + f) % F for f in range(B)]
+            t = torch.from_numpy(np.ascontiguousarray(traces[sel]))
+            if host:
+                self.tr.append(t.pin_memory())
+                self.img.append(torch.empty((B, geom.npix), dtype=torch.float32).pin_memory())
+            else:
+                self.tr.append(t.cuda())
+                self.img.append(torch.empty((B, geom.npix), dtype=torch.float32, device="cuda"))
+            self.plans.append(p)
+        self.stream = torch.cuda.Stream()
+        self.graph = None
+        torch.cuda.synchronize()
+
+    def step(self, i):
+        r = i % self.R
+        self.plans[r].backproject(self.tr[r], self.img[r], self.B, self.stream)
+
+    def capture_round(self):
+        """One CUDA graph holding one step on each of the R plans (kills the per-launch host cost)."""
+        torch = self.torch
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(self.stream):
+            with torch.cuda.graph(g, stream=self.stream):
+                for r in range(self.R):
+                    self.step(r)
+        self.graph = g
+
+    def run(self, nsteps):
+        """Enqueue exactly nsteps steps on self.stream (graph rounds + a direct-call remainder)."""
+        torch = self.torch
+        with torch.cuda.stream(self.stream):
+            q, rem = (nsteps // self.R, nsteps % self.R) if self.graph is not None else (0, nsteps)
+            for _ in range(q):
+                self.graph.replay()
+            for i in range(rem):
+                self.step(i)
+
+    def launches(self):
+        return sum(p.launches() for p in self.plans)
+
+    def close(self):
+        self.graph = None
+        for p in self.plans:
+            p.close()
+        self.plans = []
+
+
+def time_steps(rig, nsteps, warmup, dist=None):
+    """Device time (ms) of exactly nsteps steps: barrier + synchronize on both sides, CUDA events
+    on the launching stream, max over ranks."""
+    torch = rig.torch
+    rig.run(warmup)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(rig.stream)
+    rig.run(nsteps)
+    e1.record(rig.stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        dist.barrier()
+    return ms
+
+
+def profile_gather(rig, nsteps):
+    """Mean device duration (ms) of the pre-pass and of the gather kernel over nsteps direct calls,
+    from CUDA events recorded by the library on the launching stream."""
+    pat, torch = rig.pat, rig.torch
+    for p in rig.plans:
+        pat.pat_set_profiling(p.handle, 1)
+    with torch.cuda.stream(rig.stream):
+        for i in range(nsteps):
+            rig.step(i)
+    torch.cuda.synchronize()
+    n = a = b = 0.0
+    for p in rig.plans:
+        c, pa, ga = pat.pat_get_profile(p.handle, True)
+        n, a, b = n + c, a + pa, b + ga
+        pat.pat_set_profiling(p.handle, 0)
+    return (a / n, b / n) if n else (float("nan"), float("nan"))
+
+
+def measure(geom, tau, traces, B, steps, warmup, variant, dist, peak_gbs, sm_mhz, do_e2e):
+    """All device-side numbers of one (geometry, B) point."""
+    S, P, Nt = geom.nsens, geom.npix, geom.nt
+    upd = float(B) * S * P
+    abytes = algorithmic_bytes(S, P, Nt, B)
+    rig = Rig(geom, tau, traces, B, variant)
+    rig.run(rig.R)                                       # first-call set-up outside the capture
+    rig.torch.cuda.synchronize()
+    rig.capture_round()
+    l0 = rig.launches()
+    ms = time_steps(rig, steps, warmup, dist)
+    per_step_launches = 2                                # pre-pass + gather per pat_backproject
+    pre_ms, gat_ms = profile_gather(rig, min(max(steps, rig.R), 512))
+    out = {
+        "B": B, "plans_rotated": rig.R, "ms_per_step": ms / steps, "ms_per_frame": ms / steps / B,
+        "gupd_s": upd * steps / (ms * 1e-3) / 1e9,
+        "step_bytes": abytes,
+        "step_hbm_frac": abytes * steps / (ms * 1e-3) / 1e9 / peak_gbs,
+        "prepass_ms": pre_ms, "gather_ms": gat_ms,
+        "gather_gbs": abytes / (gat_ms * 1e-3) / 1e9,
+        "launches_per_step": per_step_launches,
+        "direct_call_launches_seen": rig.launches() - l0,
+    }
+    # SM-side bound: 8 B of shared-memory/L1 traffic per update at 128 B/clk/SM
+    sms = rig.torch.cuda.get_device_properties(rig.torch.cuda.current_device()).multi_processor_count
+    smem_upd_s = SMEM_BYTES_PER_CLK_SM / 8.0 * sms * sm_mhz * 1e6
+    out["sm_side_frac"] = (upd / (gat_ms * 1e-3)) / smem_upd_s
+    out["l2_bytes"] = rig.l2_bytes
+    rig.close()
+    if do_e2e:
+        hrig = Rig(geom, tau, traces, B, variant, host=True)
+        n_e2e = max(hrig.R, min(steps, 200))
+        ms_h = time_steps(hrig, n_e2e, min(warmup, 10), dist)
+        out["e2e_gupd_s"] = upd * n_e2e / (ms_h * 1e-3) / 1e9
+        out["e2e_ms_per_step"] = ms_h / n_e2e
+        out["h2d"] = 4 * B * S * Nt
+        out["d2h"] = 4 * B * P
+        hrig.close()
+    return out
+
+
+# ---------------------------------------------------------------------------------------------
+# CPU oracle legs (the only places bench.py executes oracle/)
+# ---------------------------------------------------------------------------------------------
+def oracle_time(geom, tau, traces, reps=1):
+    """Seconds per call of oracle.backproject on `traces` (as it stands: OpenMP over pixels)."""
+    import oracle
+    oracle.backproject(tau, traces[:1], geom.fs, geom.t0, 1)          # load + first touch
+    best = float("inf")
+    for _ in range(reps):
+        t = time.perf_counter()
+        oracle.backproject(tau, traces, geom.fs, geom.t0, 1)
+        best = min(best, time.perf_counter() - t)
+    return best
+
+
+def host_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def cpu_baseline(geom, tau, traces_all):
+    nf = min(16, traces_all.shape[0])
+    sample = traces_all[:nf]
+    sec = oracle_time(geom, tau, sample, reps=2)
+    upd = float(nf) * geom.nsens * geom.npix
+    return {"value": upd / sec / 1e9, "unit": "GUpd/s", "cores": host_cores(), "kind": "oracle",
+            "ms_per_frame": sec / nf * 1e3,
+            "sample": "%d seeded frames of configs[%d] geometry (S=%d, P=%d, Nt=%d), one oracle call, best of 2"
+                      % (nf, geom.k, geom.nsens, geom.npix, geom.nt)}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on the same config / metric (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    k = args.config
+    Bcfg = args.batch or W.make_geometry(k, args.reduced).batch
+    nf = min(Bcfg, 4)                                    # bounded sample: <= 4 frames per step
+    geom, tau, traces = prepare_inputs(k, args.reduced, nf)
+    for _ in range(max(1, min(args.warmup, 3))):
+        oracle_time(geom, tau, traces, reps=1)
+    t = time.perf_counter()
+    import oracle
+    for _ in range(args.steps):
+        oracle.backproject(tau, traces, geom.fs, geom.t0, 1)
+    sec = time.perf_counter() - t
+    upd = float(nf) * geom.nsens * geom.npix * args.steps
+    val = upd / sec / 1e9
+    sample = "each step = %d frame(s) of configs[%d] (S=%d, P=%d, Nt=%d) through oracle.backproject" % (
+        nf, k, geom.nsens, geom.npix, geom.nt)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "GUpd/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "gpu_launches": 0,
+        "config": {"workload": "configs[%d] %s" % (k, geom.name), "nsens": geom.nsens, "npix": geom.npix,
+                   "nt": geom.nt, "frames_per_step": nf},
+        "cpu_baseline": {"value": val, "unit": "GUpd/s", "cores": host_cores(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "GUpd/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------
+# main (the CUDA arm)
+# ---------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import paper_1501_03869_b200 as pat
+    pat.lib()                                            # fails loudly if the extension is missing
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (B200); there is no CPU fallback. "
+                         "Use --impl reference for the CPU oracle arm.")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist = dist_mod
+    peak_gbs, peak_src, sm_max = measured_peaks()
+
+    k = args.config
+    geom0 = W.make_geometry(k, args.reduced)
+    B = args.batch or geom0.batch
+    do_sweep = (not args.no_sweep) and world == 1 and k in (1, 2) and not args.batch
+    nframes = 64 if do_sweep else max(B, 16 if (world == 1 and not args.no_cpu_baseline) else B)
+    # every rank owns its own frames: the path shards over frames with no exchange (weak scaling)
+    geom, tau, traces = prepare_inputs(k, args.reduced, nframes, frame0=rank * nframes)
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    main = measure(geom, tau, traces, B, args.steps, args.warmup, args.variant, dist, peak_gbs, sm_max,
+                   not args.no_e2e)
+    clocks_main = None
+    sweep = []
+    if do_sweep:
+        for b in (1, 2, 4, 8, 16, 32, 64):
+            if b == B:
+                m = main
+            else:
+                st = max(20, min(args.steps, int(args.steps * 4 / b)))
+                m = measure(geom, tau, traces, b, st, min(args.warmup, 10), args.variant, None, peak_gbs,
+                            sm_max, False)
+            sweep.append({"B": b, "ms_per_frame": round(m["ms_per_frame"], 6),
+                          "gupd_s": round(m["gupd_s"], 1),
+                          "step_hbm_frac": round(m["step_hbm_frac"], 4),
+                          "gather_hbm_frac": round(m["gather_gbs"] / peak_gbs, 4),
+                          "sm_side_frac": round(m["sm_side_frac"], 4)})
+    sampler.stop_flag = True
+    sampler.join(timeout=2.0)
+    clocks_main = sampler.summary()
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    S, P, Nt = geom.nsens, geom.npix, geom.nt
+    gather_gbs = main["gather_gbs"]
+    line = {
+        "metric": METRIC, "value": main["gupd_s"] * world, "unit": "GUpd/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": main["ms_per_step"],
+        "ms_per_frame": main["ms_per_frame"], "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "configs[%d] %s: %d sensors x %d px, Nt=%d, %d frame(s)/step"
+                               % (k, geom.name, S, P, Nt, B),
+                   "nsens": S, "npix": P, "nt": Nt, "frames_per_step": B, "weighting": "p - t*dp/dt (Eq. 7)",
+                   "parallelism": "frames sharded over %d rank(s), no collective" % world,
+                   "l2_policy": "inputs larger than L2: %d rotating plans x %.1f MB per step vs %.0f MB L2"
+                                % (main["plans_rotated"], main["step_bytes"] / 1e6, main["l2_bytes"] / 1e6),
+                   "launch": "CUDA graph replay of pat_backproject (pre-pass + gather) per plan"},
+        "gpu_launches": int(main["launches_per_step"] * args.steps),
+        "clocks": clocks_main,
+        "roofline": {"bound": "hbm", "achieved": gather_gbs, "peak": peak_gbs, "unit": "GB/s",
+                     "frac": gather_gbs / peak_gbs, "traffic": None, "peak_source": peak_src,
+                     "kernel": "gather", "kernel_ms": main["gather_ms"], "prepass_ms": main["prepass_ms"],
+                     "algorithmic_bytes_per_launch": main["step_bytes"],
+                     "frac_of_nominal_8TBs": gather_gbs / NOMINAL_HBM_GBS,
+                     "step_frac": main["step_hbm_frac"], "sm_side_frac": main["sm_side_frac"]},
+        "paper_context": "PAPER.md:79: 123.79 ms for 512 sensors x 21323 px on a Tesla C2075, transfers included",
+    }
+    if "e2e_gupd_s" in main:
+        line["e2e"] = {"value": main["e2e_gupd_s"] * world, "unit": "GUpd/s",
+                       "h2d_bytes_per_step": main["h2d"], "d2h_bytes_per_step": main["d2h"],
+                       "ms_per_step": main["e2e_ms_per_step"]}
+    if sweep:
+        line["sweep"] = sweep
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(geom, tau, traces)
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    try:                                                 # dram bytes per gather launch from the committed ncu capture
+        with open(tpath) as f:
+            line["roofline"]["traffic"] = json.load(f).get("configs[%d]/B=%d" % (k, B))
+    except Exception:
+        pass
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    sys.exit(run_reference(a) if a.impl == "reference" else run_ours(a))

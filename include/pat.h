@@ -124,6 +124,15 @@ int64_t pat_kernel_launches(const pat_plan *plan);
  * shared memory).  PAT_ERR_UNSUPPORTED if the variant cannot run this plan. */
 pat_status pat_set_gather_variant(pat_plan *plan, int32_t variant);
 
+/* Measurement helper (bench.py's roofline leg): while enabled, pat_backproject brackets the
+ * pre-pass and the gather with CUDA events on `stream` (this disables their programmatic
+ * overlap).  pat_get_profile waits for the recorded events and returns the number of profiled
+ * calls and the summed device milliseconds of each kernel since the last reset; any out
+ * pointer may be NULL.  At most 65536 calls are recorded between resets. */
+pat_status pat_set_profiling(pat_plan *plan, int32_t enable);
+pat_status pat_get_profile(pat_plan *plan, int32_t reset, int64_t *calls, double *prepass_ms,
+                           double *gather_ms);
+
 /* pat_fmm_travel_times -- UNTIMED input preparation, HOST only: the
  * first-order upwind, heap-ordered narrow-band fast marching solve of |grad T| = 1/c from
  * each sensor (reciprocity); order = 2 uses the paper's Eq. 6 stencil with

@@ -75,6 +75,11 @@ def lib():
     L.pat_kernel_launches.argtypes = [vp]
     L.pat_set_gather_variant.restype = ctypes.c_int
     L.pat_set_gather_variant.argtypes = [vp, i32]
+    L.pat_set_profiling.restype = ctypes.c_int
+    L.pat_set_profiling.argtypes = [vp, i32]
+    L.pat_get_profile.restype = ctypes.c_int
+    L.pat_get_profile.argtypes = [vp, i32, ctypes.POINTER(i64), ctypes.POINTER(ctypes.c_double),
+                                  ctypes.POINTER(ctypes.c_double)]
     L.pat_fmm_travel_times.restype = ctypes.c_int
     L.pat_fmm_travel_times.argtypes = [gp, vp, vp, i32, vp, i64, i32, i32, i32, vp, i32]
     L.pat_compute_travel_times.restype = ctypes.c_int
@@ -156,6 +161,17 @@ def pat_kernel_launches(plan):
 
 def pat_set_gather_variant(plan, variant):
     return _check(plan, lib().pat_set_gather_variant(plan, variant))
+
+
+def pat_set_profiling(plan, enable):
+    return _check(plan, lib().pat_set_profiling(plan, int(enable)))
+
+
+def pat_get_profile(plan, reset=True):
+    """(calls, prepass_ms, gather_ms) summed since the last reset."""
+    n, a, b = ctypes.c_int64(), ctypes.c_double(), ctypes.c_double()
+    _check(plan, lib().pat_get_profile(plan, int(reset), ctypes.byref(n), ctypes.byref(a), ctypes.byref(b)))
+    return n.value, a.value, b.value
 
 
 def pat_fmm_travel_times(grid, c_map, sensor_xyz, nsens, roi_index, npix, sensor_begin, count, order,

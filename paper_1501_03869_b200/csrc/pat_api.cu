@@ -265,18 +265,30 @@ extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *i
                                         cudaMemcpyHostToDevice, st);
         if (e != cudaSuccess) return cuda_fail(p, e, "traces H2D copy");
     }
-    PatLaunchCtx ctx{stream, p->num_sms, p->use_pdl};
+    const bool prof = p->profiling && p->prof_events.size() < 3u * 65536u;
+    PatLaunchCtx ctx{stream, p->num_sms, p->use_pdl && !prof};
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    if (prof) {
+        for (int q = 0; q < 3; ++q) {
+            cudaError_t ee = cudaEventCreate(&ev[q]);
+            if (ee != cudaSuccess) return cuda_fail(p, ee, "cudaEventCreate");
+            p->prof_events.push_back(ev[q]);
+        }
+        cudaEventRecord(ev[0], st);
+    }
     float *bd = (float *)(p->ws + p->lay.bd);
     const float t0fs = (float)((double)p->t0 * (double)p->fs);
     int e = pat_launch_prepass(ctx, d_tr, bd, d_img, d.nsens, d.nt, nframes, d.npix, p->wp, p->wd, t0fs);
     if (e) return cuda_fail(p, e, "pre-pass launch");
     ++p->launches;
+    if (prof) cudaEventRecord(ev[1], st);
     if (p->variant == 2) return fail(p, PAT_ERR_UNSUPPORTED, "frame-lane gather not available for this plan");
     e = pat_launch_gather_pixel(ctx, (const float *)(p->ws + p->lay.tau), bd,
                                 (const int32_t *)(p->ws + p->lay.perm), d_img, d.nsens, d.npix, d.ntiles,
                                 d.nt, nframes, p->fs, p->t0);
     if (e) return cuda_fail(p, e, "gather launch");
     ++p->launches;
+    if (prof) cudaEventRecord(ev[2], st);
     if (!td) {
         cudaError_t ce = cudaMemcpyAsync(images, d_img, (size_t)nframes * d.npix * sizeof(float),
                                          cudaMemcpyDeviceToHost, st);
@@ -285,8 +297,41 @@ extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *i
     return PAT_OK;
 }
 
+static void drop_events(pat_plan *p) {
+    for (void *e : p->prof_events) cudaEventDestroy((cudaEvent_t)e);
+    p->prof_events.clear();
+}
+
 extern "C" pat_status pat_destroy(pat_plan *p) {
+    if (p) drop_events(p);
     delete p;
+    return PAT_OK;
+}
+
+extern "C" pat_status pat_set_profiling(pat_plan *p, int32_t enable) {
+    if (!p) return PAT_ERR_INVALID_ARG;
+    p->profiling = enable != 0;
+    return PAT_OK;
+}
+
+extern "C" pat_status pat_get_profile(pat_plan *p, int32_t reset, int64_t *calls, double *prepass_ms,
+                                      double *gather_ms) {
+    if (!p) return PAT_ERR_INVALID_ARG;
+    double a = 0.0, b = 0.0;
+    const size_t n = p->prof_events.size() / 3;
+    for (size_t q = 0; q < n; ++q) {
+        cudaEvent_t *ev = (cudaEvent_t *)&p->prof_events[3 * q];
+        cudaError_t e = cudaEventSynchronize(ev[2]);
+        float m0 = 0.f, m1 = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&m0, ev[0], ev[1]);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&m1, ev[1], ev[2]);
+        if (e != cudaSuccess) return cuda_fail(p, e, "profile events");
+        a += m0; b += m1;
+    }
+    if (calls) *calls = (int64_t)n;
+    if (prepass_ms) *prepass_ms = a;
+    if (gather_ms) *gather_ms = b;
+    if (reset) drop_events(p);
     return PAT_OK;
 }
 
