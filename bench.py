@@ -57,8 +57,12 @@ def parse_args():
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--variant", type=int, default=0, help="pat_set_gather_variant (0 = automatic)")
+    ap.add_argument("--tuning", type=str, default="", help="wr,rows,stages for pat_set_gather_tuning (0 = automatic)")
     return ap.parse_args()
+
+
+def tuning_of(args):
+    return tuple(int(v) for v in args.tuning.split(",")) if args.tuning else None
 
 
 def measured_peaks():
@@ -163,7 +167,7 @@ class Rig:
             p = pat.Plan(geom.n, geom.h, geom.origin, None, geom.sensors, geom.roi_index, geom.nt, geom.fs,
                          geom.t0, weighting=pat.PAT_W_PAPER, max_batch=B)
             if variant:
-                pat.pat_set_gather_variant(p.handle, variant)
+                pat.pat_set_gather_tuning(p.handle, *variant)
             p.set_travel_times(tau)
             sel = [(r * B + f) % F for f in range(B)]
             t = torch.from_numpy(np.ascontiguousarray(traces[sel]))
@@ -392,7 +396,7 @@ def run_ours(args):
 
     sampler = ClockSampler(local)
     sampler.start()
-    main = measure(geom, tau, traces, B, args.steps, args.warmup, args.variant, dist, peak_gbs, sm_max,
+    main = measure(geom, tau, traces, B, args.steps, args.warmup, tuning_of(args), dist, peak_gbs, sm_max,
                    not args.no_e2e)
     clocks_main = None
     sweep = []
@@ -402,7 +406,7 @@ def run_ours(args):
                 m = main
             else:
                 st = max(20, min(args.steps, int(args.steps * 4 / b)))
-                m = measure(geom, tau, traces, b, st, min(args.warmup, 10), args.variant, None, peak_gbs,
+                m = measure(geom, tau, traces, b, st, min(args.warmup, 10), tuning_of(args), None, peak_gbs,
                             sm_max, False)
             sweep.append({"B": b, "ms_per_frame": round(m["ms_per_frame"], 6),
                           "gupd_s": round(m["gupd_s"], 1),

@@ -54,9 +54,9 @@ typedef struct {
 } pat_grid;
 
 /* Bytes of DEVICE workspace a plan with these sizes needs (0 on invalid sizes).
- * Layout: re-tiled tau table (the dominant term, 4*nsens*npix rounded up to whole
- * 256-pixel tiles), weighted traces for max_batch frames, staging for host-side
- * inputs, pixel permutation. */
+ * Layout: re-tiled table (the dominant term, 4*nsens*npix rounded up to whole
+ * 256-pixel tiles), per-row sample ranges, weighted traces for max_batch frames (rounded up to
+ * the frame-count class), staging for host-side inputs, pixel permutation. */
 size_t pat_plan_workspace_bytes(const pat_grid *grid, int32_t nsens, int64_t npix,
                                 int32_t nt, int32_t max_batch);
 
@@ -87,9 +87,10 @@ pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, const float *c_
 /* pat_set_travel_times -- hand the plan rows of the tau table.
  *   tau   fp32 seconds, row-major [count][npix] (pixel order = roi_index order) for sensors
  *         [sensor_begin, sensor_begin+count).  HOST or DEVICE pointer (detected).
- * Copies and re-tiles the rows into the workspace (spatially compact 256-pixel tiles) on
- * `stream`; a host source is staged in pieces, so the call returns after the host buffer has
- * been consumed.  May be called repeatedly with disjoint sensor ranges (the 34 GB 3-D table).
+ * Converts to sample units u = fl32(fl32(tau - t0)*fs) and re-tiles the rows into the workspace
+ * (spatially compact 256-pixel tiles) on `stream`; a host source is staged in pieces, so the call
+ * returns after the host buffer has been consumed.  The call that completes the table (every
+ * sensor row set) also reduces each (tile, sensor) row to its sample range and synchronises.  May be called repeatedly with disjoint sensor ranges (the 34 GB 3-D table).
  * Values that are negative, NaN, +-inf or beyond the record are LEGAL and contribute 0. */
 pat_status pat_set_travel_times(pat_plan *plan, const float *tau, int32_t sensor_begin,
                                 int32_t count, void *stream);
@@ -101,7 +102,10 @@ pat_status pat_set_travel_times(pat_plan *plan, const float *tau, int32_t sensor
  *   traces  fp32 [nframes][nsens][nt]     images  fp32 [nframes][npix] (roi_index order)
  * Both DEVICE (16-byte aligned) or both HOST pointers (detected; host buffers should be
  * pinned for the copies to be asynchronous).  Enqueues weighting pre-pass + gather (+ the
- * copies for host buffers) on `stream` and returns without synchronising.
+ * copies for host buffers) on `stream` and returns without synchronising -- except for the first
+ * call with a given frame-count class (1, 2, 3-4, 5-8, ..., 33+) after the table changed, which
+ * builds that class's work list (a few hundred KB of library-owned device memory, freed by
+ * pat_destroy) and must therefore not happen inside a stream capture.
  * nframes = 0 is a no-op; nframes > max_batch -> PAT_ERR_INVALID_ARG; tau rows missing ->
  * PAT_ERR_BAD_STATE. */
 pat_status pat_backproject(pat_plan *plan, const float *traces, float *images,
@@ -119,10 +123,14 @@ const char *pat_last_error(const pat_plan *plan);
 /* Number of kernels of this library launched through `plan` so far (monotone counter). */
 int64_t pat_kernel_launches(const pat_plan *plan);
 
-/* Select the gather implementation: 0 = automatic, 1 = pixel-lane (one thread per pixel,
- * traces gathered through L1), 2 = frame-lane (lanes = frames, trace windows staged in
- * shared memory).  PAT_ERR_UNSUPPORTED if the variant cannot run this plan. */
-pat_status pat_set_gather_variant(pat_plan *plan, int32_t variant);
+/* Override the gather's shared-memory geometry (tuning / test hook; 0 = choose automatically):
+ *   wr      window ring in samples, a power of two in [8, 4096]: a (tile, sensor) row whose pixels
+ *           span more than wr-4 samples of the trace is processed in several segments;
+ *   rows    (tile, sensor) rows per pipeline stage, 1..32;   stages  pipeline depth, 2..8.
+ * A request that does not fit one CTA's shared memory for a given frame-count class is shrunk
+ * (rows, then stages, then wr).  Takes effect at the next pat_backproject (the work lists are
+ * rebuilt).  Results do not depend on the tuning beyond fp32 summation order. */
+pat_status pat_set_gather_tuning(pat_plan *plan, int32_t wr, int32_t rows, int32_t stages);
 
 /* Measurement helper (bench.py's roofline leg): while enabled, pat_backproject brackets the
  * pre-pass and the gather with CUDA events on `stream` (this disables their programmatic

@@ -73,8 +73,8 @@ def lib():
     L.pat_last_error.argtypes = [vp]
     L.pat_kernel_launches.restype = i64
     L.pat_kernel_launches.argtypes = [vp]
-    L.pat_set_gather_variant.restype = ctypes.c_int
-    L.pat_set_gather_variant.argtypes = [vp, i32]
+    L.pat_set_gather_tuning.restype = ctypes.c_int
+    L.pat_set_gather_tuning.argtypes = [vp, i32, i32, i32]
     L.pat_set_profiling.restype = ctypes.c_int
     L.pat_set_profiling.argtypes = [vp, i32]
     L.pat_get_profile.restype = ctypes.c_int
@@ -159,8 +159,8 @@ def pat_kernel_launches(plan):
     return int(lib().pat_kernel_launches(plan))
 
 
-def pat_set_gather_variant(plan, variant):
-    return _check(plan, lib().pat_set_gather_variant(plan, variant))
+def pat_set_gather_tuning(plan, wr=0, rows=0, stages=0):
+    return _check(plan, lib().pat_set_gather_tuning(plan, wr, rows, stages))
 
 
 def pat_set_profiling(plan, enable):

@@ -70,6 +70,124 @@ inline uint64_t spread3(uint32_t v) {
     return x;
 }
 
+void drop_schedules(pat_plan *p) {
+    for (PatSchedule &sc : p->schedules) {
+        if (sc.d_sched) cudaFree(sc.d_sched);
+        if (sc.d_cta_chunk) cudaFree(sc.d_cta_chunk);
+    }
+    p->schedules.clear();
+}
+
+// The table is complete: reduce every (tile, sensor) row to its k-range and keep a host copy,
+// from which the per-configuration work lists are built (build_schedule).  Synchronises `stream`.
+pat_status finalize_table(pat_plan *p, void *stream) {
+    const int64_t nrows = p->dims.ntiles * p->dims.nsens;
+    PatLaunchCtx ctx{stream, p->num_sms, false};
+    int e = pat_launch_row_meta(ctx, (const float *)(p->ws + p->lay.tau), p->ws + p->lay.meta, nrows, p->dims.nt);
+    if (e) return cuda_fail(p, e, "row-meta launch");
+    ++p->launches;
+    try { p->host_meta.resize((size_t)nrows * 2); } catch (...) { return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
+    cudaError_t ce = cudaMemcpyAsync(p->host_meta.data(), p->ws + p->lay.meta, (size_t)nrows * 2 * sizeof(int32_t),
+                                     cudaMemcpyDeviceToHost, (cudaStream_t)stream);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize((cudaStream_t)stream);
+    if (ce != cudaSuccess) return cuda_fail(p, ce, "row-meta read-back");
+    p->meta_valid = true;
+    return PAT_OK;
+}
+
+struct Desc { int32_t tile, sensor, s0, w; };
+
+// Work list for one shared-memory geometry: every row is cut into segments of at most wr-4
+// k-values (one descriptor each; rows without a valid pixel vanish), the descriptors are dealt
+// to grid_x persistent CTAs in equal shares and grouped into chunks of exactly R (null-padded);
+// a chunk never mixes tiles.  Bit 30 of w marks a chunk whose R descriptors are all whole rows.
+pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule **out) {
+    const int64_t ntiles = p->dims.ntiles;
+    const int32_t S = p->dims.nsens;
+    const int32_t step = cfg.wr - 4, R = cfg.R;
+    const int32_t *meta = p->host_meta.data();
+    int64_t V = 0;
+    for (int64_t r = 0; r < ntiles * S; ++r) {
+        const int32_t kmin = meta[2 * r], kmax = meta[2 * r + 1];
+        if (kmax >= kmin) V += (kmax + 1 - (kmin & ~3) + step - 1) / step;
+    }
+    PatSchedule sc;
+    sc.cfg = cfg;
+    int per_sm = 0;
+    int e = pat_gather_occupancy(cfg, &per_sm);
+    if (e) return cuda_fail(p, e, "gather occupancy query");
+    if (per_sm < 1) return fail(p, PAT_ERR_CUDA, "gather kernel does not fit on an SM with this tuning");
+    int64_t G = (int64_t)p->num_sms * per_sm;
+    G = std::min<int64_t>(G, (V + R - 1) / R);
+    sc.grid_x = (int)G;
+    if (V == 0) { p->schedules.push_back(sc); *out = &p->schedules.back(); return PAT_OK; }
+    std::vector<Desc> list;
+    std::vector<int32_t> cta_chunk;
+    try {
+        list.reserve((size_t)(V + (ntiles + G) * R));
+        cta_chunk.reserve((size_t)G + 1);
+        int64_t vi = 0, c = 0, vend = V / G;       // CTA c owns virtual rows [V*c/G, V*(c+1)/G)
+        size_t open = 0;                           // first descriptor of the open chunk
+        bool simple = true;
+        cta_chunk.push_back(0);
+        auto close_chunk = [&]() {
+            if (list.size() == open) return;
+            if (list.size() - open < (size_t)R) simple = false;
+            const int32_t tile = list[open].tile;
+            while (list.size() - open < (size_t)R) list.push_back(Desc{tile, 0, 0, 0});
+            if (simple) for (size_t q = open; q < list.size(); ++q) list[q].w |= 1 << 30;
+            open = list.size();
+            simple = true;
+        };
+        for (int64_t t = 0; t < ntiles; ++t) {
+            for (int32_t s = 0; s < S; ++s) {
+                const int64_t r = t * S + s;
+                const int32_t kmin = meta[2 * r], kmax = meta[2 * r + 1];
+                if (kmax < kmin) continue;
+                const int32_t n0 = kmin & ~3, kend = kmax + 1;
+                const bool whole = kend - n0 <= step;
+                for (int32_t s0 = n0; s0 < kend; s0 += step) {
+                    if (vi == vend && c + 1 < G) {         // next CTA's share begins
+                        close_chunk();
+                        cta_chunk.push_back((int32_t)(list.size() / R));
+                        ++c;
+                        vend = V * (c + 1) / G;
+                    }
+                    if (list.size() > open && list[open].tile != (int32_t)t) close_chunk();
+                    list.push_back(Desc{(int32_t)t, s, s0, std::min(step, kend - s0)});
+                    if (!whole) simple = false;
+                    if (list.size() - open == (size_t)R) close_chunk();
+                    ++vi;
+                }
+            }
+        }
+        close_chunk();
+        while ((int64_t)cta_chunk.size() < G + 1) cta_chunk.push_back((int32_t)(list.size() / R));
+    } catch (...) { return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
+    if (list.size() / R > (size_t)INT32_MAX) return fail(p, PAT_ERR_UNSUPPORTED, "work list too long");
+    sc.nchunks = (int64_t)(list.size() / R);
+    cudaError_t ce = cudaMalloc(&sc.d_sched, list.size() * sizeof(Desc));
+    if (ce == cudaSuccess) ce = cudaMalloc((void **)&sc.d_cta_chunk, cta_chunk.size() * sizeof(int32_t));
+    if (ce == cudaSuccess) ce = cudaMemcpy(sc.d_sched, list.data(), list.size() * sizeof(Desc), cudaMemcpyHostToDevice);
+    if (ce == cudaSuccess)
+        ce = cudaMemcpy(sc.d_cta_chunk, cta_chunk.data(), cta_chunk.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (ce != cudaSuccess) {
+        if (sc.d_sched) cudaFree(sc.d_sched);
+        if (sc.d_cta_chunk) cudaFree(sc.d_cta_chunk);
+        return cuda_fail(p, ce, "work-list upload");
+    }
+    p->schedules.push_back(sc);
+    *out = &p->schedules.back();
+    return PAT_OK;
+}
+
+pat_status get_schedule(pat_plan *p, int bp, PatSchedule **out) {
+    for (PatSchedule &sc : p->schedules)
+        if (sc.cfg.bp == bp) { *out = &sc; return PAT_OK; }
+    PatGatherConfig cfg = pat_gather_config(bp, p->tune_wr, p->tune_R, p->tune_stages);
+    return build_schedule(p, cfg, out);
+}
+
 }  // namespace
 
 PatLayout pat_layout(const PatDims &d) {
@@ -77,7 +195,10 @@ PatLayout pat_layout(const PatDims &d) {
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
     L.tau = take((size_t)d.ntiles * d.nsens * kTilePix * sizeof(float));
-    L.bd = take((size_t)d.max_batch * d.nsens * d.nt * 2 * sizeof(float));
+    L.meta = take((size_t)d.ntiles * d.nsens * 2 * sizeof(int32_t));
+    const int bp = pat_frames_per_group(d.max_batch);
+    const size_t padded = (size_t)(d.max_batch + bp - 1) / bp * bp;
+    L.bd = take(padded * d.nsens * ((d.nt + 3) / 4 * 4) * sizeof(float));
     L.perm = take((size_t)d.ntiles * kTilePix * sizeof(int32_t));
     L.traces = take((size_t)d.max_batch * d.nsens * d.nt * sizeof(float));
     L.images = take((size_t)d.max_batch * d.npix * sizeof(float));
@@ -145,6 +266,7 @@ extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, cons
     p->grid = *grid;
     if (grid->ndim == 2) { p->grid.n[2] = 1; p->grid.origin[2] = 0.0f; }
     p->fs = fs; p->t0 = t0; p->weighting = weighting;
+    p->nt4 = (nt + 3) / 4 * 4;
     p->wp = weighting == PAT_W_UBP ? 2.0f : 1.0f;
     p->wd = weighting == PAT_W_DELAY_SUM ? 0.0f : p->wp;
     p->ws = (char *)workspace;
@@ -214,7 +336,8 @@ extern "C" pat_status pat_set_travel_times(pat_plan *p, const float *tau, int32_
     const int32_t *perm = (const int32_t *)(p->ws + p->lay.perm);
     const int64_t P = p->dims.npix;
     if (on_dev) {
-        int e = pat_launch_retile(ctx, tau, tau_t, perm, p->dims.nsens, P, p->dims.ntiles, sensor_begin, count);
+        int e = pat_launch_retile(ctx, tau, tau_t, perm, p->dims.nsens, P, p->dims.ntiles, sensor_begin, count,
+                                  p->fs, p->t0);
         if (e) return cuda_fail(p, e, "retile launch");
         ++p->launches;
     } else {
@@ -225,7 +348,7 @@ extern "C" pat_status pat_set_travel_times(pat_plan *p, const float *tau, int32_
                                             cudaMemcpyHostToDevice, st);
             if (e != cudaSuccess) return cuda_fail(p, e, "tau H2D copy");
             int le = pat_launch_retile(ctx, stage, tau_t, perm, p->dims.nsens, P, p->dims.ntiles,
-                                       sensor_begin + r, m);
+                                       sensor_begin + r, m, p->fs, p->t0);
             if (le) return cuda_fail(p, le, "retile launch");
             ++p->launches;
             // the staging buffer is reused by the next piece and the host rows are only
@@ -236,6 +359,9 @@ extern "C" pat_status pat_set_travel_times(pat_plan *p, const float *tau, int32_
     }
     for (int32_t s = sensor_begin; s < sensor_begin + count; ++s)
         if (!p->row_set[s]) { p->row_set[s] = 1; ++p->rows_set; }
+    p->meta_valid = false;
+    drop_schedules(p);
+    if (p->rows_set == p->dims.nsens) return finalize_table(p, stream);
     return PAT_OK;
 }
 
@@ -265,6 +391,12 @@ extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *i
                                         cudaMemcpyHostToDevice, st);
         if (e != cudaSuccess) return cuda_fail(p, e, "traces H2D copy");
     }
+    const int bp = pat_frames_per_group(nframes);
+    PatSchedule *sc = nullptr;
+    {   // first use of this frame-count class after the table changed: builds the work list (synchronous)
+        pat_status ss = get_schedule(p, bp, &sc);
+        if (ss != PAT_OK) return ss;
+    }
     const bool prof = p->profiling && p->prof_events.size() < 3u * 65536u;
     PatLaunchCtx ctx{stream, p->num_sms, p->use_pdl && !prof};
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
@@ -276,18 +408,19 @@ extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *i
         }
         cudaEventRecord(ev[0], st);
     }
-    float *bd = (float *)(p->ws + p->lay.bd);
+    float *bw = (float *)(p->ws + p->lay.bd);
     const float t0fs = (float)((double)p->t0 * (double)p->fs);
-    int e = pat_launch_prepass(ctx, d_tr, bd, d_img, d.nsens, d.nt, nframes, d.npix, p->wp, p->wd, t0fs);
+    int e = pat_launch_prepass(ctx, d_tr, bw, d_img, d.nsens, d.nt, p->nt4, nframes, bp, d.npix, p->wp, p->wd, t0fs);
     if (e) return cuda_fail(p, e, "pre-pass launch");
     ++p->launches;
     if (prof) cudaEventRecord(ev[1], st);
-    if (p->variant == 2) return fail(p, PAT_ERR_UNSUPPORTED, "frame-lane gather not available for this plan");
-    e = pat_launch_gather_pixel(ctx, (const float *)(p->ws + p->lay.tau), bd,
-                                (const int32_t *)(p->ws + p->lay.perm), d_img, d.nsens, d.npix, d.ntiles,
-                                d.nt, nframes, p->fs, p->t0);
-    if (e) return cuda_fail(p, e, "gather launch");
-    ++p->launches;
+    if (sc->grid_x > 0) {
+        e = pat_launch_gather(ctx, sc->cfg, (const float *)(p->ws + p->lay.tau), bw, sc->d_sched, sc->d_cta_chunk,
+                              sc->grid_x, (const int32_t *)(p->ws + p->lay.perm), d_img, d.nsens, d.npix, d.nt,
+                              p->nt4, nframes);
+        if (e) return cuda_fail(p, e, "gather launch");
+        ++p->launches;
+    }
     if (prof) cudaEventRecord(ev[2], st);
     if (!td) {
         cudaError_t ce = cudaMemcpyAsync(images, d_img, (size_t)nframes * d.npix * sizeof(float),
@@ -303,7 +436,7 @@ static void drop_events(pat_plan *p) {
 }
 
 extern "C" pat_status pat_destroy(pat_plan *p) {
-    if (p) drop_events(p);
+    if (p) { drop_events(p); drop_schedules(p); }
     delete p;
     return PAT_OK;
 }
@@ -341,11 +474,13 @@ extern "C" const char *pat_last_error(const pat_plan *p) {
 
 extern "C" int64_t pat_kernel_launches(const pat_plan *p) { return p ? p->launches : 0; }
 
-extern "C" pat_status pat_set_gather_variant(pat_plan *p, int32_t variant) {
+extern "C" pat_status pat_set_gather_tuning(pat_plan *p, int32_t wr, int32_t rows, int32_t stages) {
     if (!p) return PAT_ERR_INVALID_ARG;
-    if (variant < 0 || variant > 2) return fail(p, PAT_ERR_INVALID_ARG, "variant must be 0, 1 or 2");
-    if (variant == 2) return fail(p, PAT_ERR_UNSUPPORTED, "frame-lane gather not available for this plan");
-    p->variant = variant;
+    if (wr < 0 || rows < 0 || stages < 0 || rows > 32 || stages > 8 || (wr && (wr < 8 || wr > 4096 || (wr & (wr - 1)))))
+        return fail(p, PAT_ERR_INVALID_ARG, "wr: 0 or a power of two in [8, 4096]; rows: 0..32; stages: 0..8");
+    if (stages == 1) return fail(p, PAT_ERR_INVALID_ARG, "stages must be 0 or >= 2");
+    p->tune_wr = wr; p->tune_R = rows; p->tune_stages = stages;
+    drop_schedules(p);
     return PAT_OK;
 }
 

@@ -27,8 +27,9 @@ struct PatDims {
 };
 
 struct PatLayout {            // byte offsets into the caller's workspace
-    size_t tau = 0;           // float  [ntiles][nsens][256]
-    size_t bd = 0;            // float2 [nsens][nt][nframes]      {b[n], b[n+1]-b[n]}
+    size_t tau = 0;           // float  [ntiles][nsens][256]   u = fl32(fl32(tau - t0)*fs), tile-major
+    size_t meta = 0;          // int2   [ntiles*nsens]         {kmin, kmax} of each row
+    size_t bd = 0;            // float  [ngroups][nsens][nt4][Bp]  weighted traces b
     size_t perm = 0;          // int32  [ntiles*256]  slot -> position in roi list, -1 = pad
     size_t traces = 0;        // float  [max_batch][nsens][nt]    staging for host traces
     size_t images = 0;        // float  [max_batch][npix]         staging for host images
@@ -39,20 +40,42 @@ struct PatLayout {            // byte offsets into the caller's workspace
 
 PatLayout pat_layout(const PatDims &d);
 
+// Shared-memory geometry of the gather for Bp frames per launch group (gather.cu).
+struct PatGatherConfig {
+    int bp = 0;               // frames per group: 1, 2, 4, ..., 64
+    int wr = 0;               // window ring, samples (power of two)
+    int R = 0;                // descriptor slots per stage
+    int stages = 0;
+    uint32_t hdr_bytes = 0, slot_bytes = 0, stage_bytes = 0;
+};
+
+// Host-built work list of one PatGatherConfig (built lazily, library-owned device memory).
+struct PatSchedule {
+    PatGatherConfig cfg;
+    int grid_x = 0;
+    int64_t nchunks = 0;
+    void *d_sched = nullptr;          // int4 [nchunks][R]
+    int32_t *d_cta_chunk = nullptr;   // int32 [grid_x + 1]
+};
+
 struct pat_plan {
     PatDims dims;
     PatLayout lay;
     pat_grid grid{};
     float fs = 0, t0 = 0;
+    int32_t nt4 = 0;
     int32_t weighting = 1;
     float wp = 1, wd = 1;
     char *ws = nullptr;       // device workspace base (borrowed)
     int device = 0;
     int num_sms = 0;
-    int variant = 0;          // 0 auto, 1 pixel-lane, 2 frame-lane
+    int tune_wr = 0, tune_R = 0, tune_stages = 0;   // pat_set_gather_tuning overrides (0 = automatic)
     bool use_pdl = true;
     std::vector<uint8_t> row_set;     // per sensor: tau row uploaded?
     int64_t rows_set = 0;
+    bool meta_valid = false;          // host_meta matches the uploaded table
+    std::vector<int32_t> host_meta;   // {kmin, kmax} per row, host copy
+    std::vector<PatSchedule> schedules;
     std::vector<float> c_map;         // host copies for pat_compute_travel_times
     std::vector<float> sensors;
     std::vector<int64_t> roi;         // empty => all nodes
@@ -69,20 +92,28 @@ struct PatLaunchCtx {
     bool use_pdl;
 };
 
-// tau rows [sensor_begin, +count) from src[count][npix] (device) into tau_t.
-int pat_launch_retile(const PatLaunchCtx &ctx, const float *src, float *tau_t, const int32_t *perm,
-                      int32_t nsens, int64_t npix, int64_t ntiles, int32_t sensor_begin, int32_t count);
+// tau rows [sensor_begin, +count) from src[count][npix] (device) -> u_t (tile-major, u = (tau-t0)*fs).
+int pat_launch_retile(const PatLaunchCtx &ctx, const float *src, float *u_t, const int32_t *perm,
+                      int32_t nsens, int64_t npix, int64_t ntiles, int32_t sensor_begin, int32_t count,
+                      float fs, float t0);
+
+// {kmin, kmax} of every row of u_t (int2 [nrows]).
+int pat_launch_row_meta(const PatLaunchCtx &ctx, const float *u_t, void *meta, int64_t nrows, int32_t nt);
 
 // H1: weighting pre-pass (Eq. 7 integrand at the sample times):
-//   traces[f][s][n] (fp32) -> bd[(s*nt + n)*nframes + f] = { b[n], b[n+1]-b[n] } (float2),
-//   entry n = nt-1 is {0,0}.  Also zeroes images[nframes*npix] (the gather accumulates into it).
-int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *bd, float *images,
-                       int32_t nsens, int32_t nt, int32_t nframes, int64_t npix,
+//   traces[f][s][n] (fp32) -> b[((g*nsens + s)*nt4 + n)*bp + fl],  f = g*bp + fl; rows n >= nt and
+//   frames f >= nframes are zero.  Also zeroes images[nframes*npix] (the gather accumulates into it).
+int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, float *images,
+                       int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp, int64_t npix,
                        float wp, float wd, float t0fs);
 
-// H2-H4: the gather, pixel-lane variant (one thread per pixel, FB frames in registers).
-int pat_launch_gather_pixel(const PatLaunchCtx &ctx, const float *tau_t, const float *bd,
-                            const int32_t *perm, float *images, int32_t nsens, int64_t npix,
-                            int64_t ntiles, int32_t nt, int32_t nframes, float fs, float t0);
+// H2-H4: the gather (gather.cu).
+int pat_frames_per_group(int32_t nframes);
+PatGatherConfig pat_gather_config(int bp, int wr, int R, int stages);   // 0 = choose automatically
+size_t pat_gather_smem_bytes(const PatGatherConfig &c);
+int pat_gather_occupancy(const PatGatherConfig &c, int *per_sm);
+int pat_launch_gather(const PatLaunchCtx &ctx, const PatGatherConfig &c, const float *u_t, const float *b,
+                      const void *sched, const int32_t *cta_chunk, int grid_x, const int32_t *perm,
+                      float *images, int32_t nsens, int64_t npix, int32_t nt, int32_t nt4, int32_t nframes);
 
 #endif  // PAT_INTERNAL_H_

@@ -1,133 +1,107 @@
-// prepass.cu -- tau re-tiling (set-up) and the H1 weighting pre-pass (sm_100a).
+// prepass.cu -- table re-tiling (set-up) and the H1 weighting pre-pass (sm_100a).
 //
 // H1 (Eq. 7): the integrand p_i(t) - t*dp_i/dt evaluated at the sample times,
 //   b[n] = wp*p[n] - wd*(n + t0*fs)*D[n],  D = central difference (one-sided at the ends),
-// stored together with its forward difference so that the gather's linear interpolation
-// (1-a)*b[k] + a*b[k+1] = b[k] + a*(b[k+1]-b[k]) is ONE 8-byte load and two FP ops.
+// written frame-fastest, b[group][sensor][sample][Bp], so that the window of samples a pixel tile
+// can touch is ONE contiguous run for all frames of a group (a single bulk async copy in gather.cu).
 #include "pat_internal.h"
 
 #include <cuda_runtime.h>
 
 namespace {
 
-// ---- tau re-tiling: row-major [count][npix] -> tile-major [tile][sensor][256] -----------
+// ---- table re-tiling: tau row-major [count][npix] -> u tile-major [tile][sensor][256] --------
+// u = fl32(fl32(tau - t0)*fs): H2's time -> sample mapping, two fp32 roundings (R8),
+// done once here instead of once per frame in the gather; padding lanes get u = -1 (invalid).
 __global__ void __launch_bounds__(256)
-retile_kernel(const float *__restrict__ src, float *__restrict__ tau_t,
+retile_kernel(const float *__restrict__ src, float *__restrict__ u_t,
               const int32_t *__restrict__ perm, int32_t nsens, int64_t npix,
-              int32_t sensor_begin, int32_t count) {
+              int32_t sensor_begin, int32_t count, float fs, float t0) {
     const int64_t tile = blockIdx.x;
     const int32_t slot = perm[tile * kTilePix + threadIdx.x];
     for (int32_t r = blockIdx.y; r < count; r += gridDim.y) {
         float v = PAT_TAU_PAD;
-        if (slot >= 0) v = __ldg(src + (int64_t)r * npix + slot);
-        tau_t[(tile * nsens + sensor_begin + r) * kTilePix + threadIdx.x] = v;
+        if (slot >= 0) v = __fmul_rn(__fsub_rn(__ldg(src + (int64_t)r * npix + slot), t0), fs);
+        u_t[(tile * nsens + sensor_begin + r) * kTilePix + threadIdx.x] = v;
     }
 }
 
-// ---- H1 -------------------------------------------------------------------------------
-// b[n] for one trace (fp32).  p points at sample 0 of the trace.
-__device__ __forceinline__ float weight_at(const float *__restrict__ p, int32_t n, int32_t nt,
-                                           float wp, float wd, float t0fs) {
-    const float pn = __ldg(p + n);
-    if (wd == 0.0f) return wp * pn;
-    float D;
-    if (n == 0)            D = __fsub_rn(__ldg(p + 1), pn);
-    else if (n == nt - 1)  D = __fsub_rn(pn, __ldg(p + n - 1));
-    else                   D = 0.5f * __fsub_rn(__ldg(p + n + 1), __ldg(p + n - 1));
-    const float tn = __fadd_rn((float)n, t0fs);
-    // wp*(p - tn*D): one rounding in the fma; wp = wd is 1 or 2 (exact scaling).
-    return wp * __fmaf_rn(-tn, D, pn);
-}
-
-// Single-frame layout: thread per sample, fully coalesced 4-byte reads / 8-byte writes.
+// ---- H1 -----------------------------------------------------------------------------------
+// Block = (sample chunk, sensor, frame group).  The chunk of every frame of the group is read
+// coalesced along time into shared memory (+1 halo each side), then written frame-fastest.
 __global__ void __launch_bounds__(256)
-prepass_b1_kernel(const float *__restrict__ traces, float2 *__restrict__ bd,
-                  float *__restrict__ images, int64_t total /* nsens*nt */, int32_t nt,
-                  int64_t npix, float wp, float wd, float t0fs) {
-#if __CUDA_ARCH__ >= 900
+prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
+               int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t log2_bp, int32_t ns,
+               int64_t npix, float wp, float wd, float t0fs) {
     asm volatile("griddepcontrol.launch_dependents;");
-#endif
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    const int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    for (int64_t q = gid; q < npix; q += stride) images[q] = 0.0f;
-    for (int64_t q = gid; q < total; q += stride) {
-        const int64_t s = q / nt;
-        const int32_t n = (int32_t)(q - s * nt);
-        const float *p = traces + s * nt;
-        float2 out = make_float2(0.0f, 0.0f);
-        if (n < nt - 1) {
-            const float b0 = weight_at(p, n, nt, wp, wd, t0fs);
-            const float b1 = weight_at(p, n + 1, nt, wp, wd, t0fs);
-            out = make_float2(b0, __fsub_rn(b1, b0));
-        }
-        bd[q] = out;
-    }
-}
-
-// Batched layout bd[(s*nt + n)*B + f]: a block handles 32 samples x all frames of one sensor;
-// frames are the fastest thread index so the 8-byte stores of a (s, n) row are contiguous.
-__global__ void __launch_bounds__(256)
-prepass_batch_kernel(const float *__restrict__ traces, float2 *__restrict__ bd,
-                     float *__restrict__ images, int32_t nsens, int32_t nt, int32_t nframes,
-                     int64_t npix, float wp, float wd, float t0fs) {
-#if __CUDA_ARCH__ >= 900
-    asm volatile("griddepcontrol.launch_dependents;");
-#endif
+    extern __shared__ float tile[];                        // [bp][ns + 3]
+    const int32_t bp = 1 << log2_bp, pitch = ns + 3;
+    const int32_t s = blockIdx.y, grp = blockIdx.z;
+    const int32_t n_begin = blockIdx.x * ns;
     {
-        const int64_t stride = (int64_t)gridDim.x * gridDim.y * blockDim.x;
-        const int64_t gid = ((int64_t)blockIdx.y * gridDim.x + blockIdx.x) * blockDim.x + threadIdx.x;
-        for (int64_t q = gid; q < npix * nframes; q += stride) images[q] = 0.0f;
+        const int64_t nblk = (int64_t)gridDim.x * gridDim.y * gridDim.z;
+        const int64_t blk = ((int64_t)grp * gridDim.y + s) * gridDim.x + blockIdx.x;
+        const int64_t tot = npix * nframes;
+        for (int64_t q = blk * 256 + threadIdx.x; q < tot; q += nblk * 256) images[q] = 0.0f;
     }
-    const int32_t s = blockIdx.y;
-    const int64_t row_elems = (int64_t)nt * nframes;
-    for (int64_t e0 = (int64_t)blockIdx.x * blockDim.x; e0 < row_elems; e0 += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t e = e0 + threadIdx.x;
-        if (e >= row_elems) break;
-        const int32_t n = (int32_t)(e / nframes);
-        const int32_t f = (int32_t)(e - (int64_t)n * nframes);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int32_t fl = warp; fl < bp; fl += 8) {
+        const int32_t f = grp * bp + fl;
         const float *p = traces + ((int64_t)f * nsens + s) * nt;
-        float2 out = make_float2(0.0f, 0.0f);
-        if (n < nt - 1) {
-            const float b0 = weight_at(p, n, nt, wp, wd, t0fs);
-            const float b1 = weight_at(p, n + 1, nt, wp, wd, t0fs);
-            out = make_float2(b0, __fsub_rn(b1, b0));
+        for (int32_t j = lane; j < ns + 2; j += 32) {
+            const int32_t n = n_begin - 1 + j;
+            tile[fl * pitch + j] = (f < nframes && n >= 0 && n < nt) ? __ldg(p + n) : 0.0f;
         }
-        bd[(int64_t)s * row_elems + e] = out;
+    }
+    __syncthreads();
+    float *out = b + (((int64_t)grp * nsens + s) * nt4 + n_begin) * bp;
+    const int32_t nloc = min(ns, nt4 - n_begin);
+    for (int32_t idx = threadIdx.x; idx < (nloc << log2_bp); idx += 256) {
+        const int32_t nl = idx >> log2_bp, fl = idx & (bp - 1);
+        const int32_t n = n_begin + nl;
+        float v = 0.0f;
+        if (n < nt && grp * bp + fl < nframes) {
+            const float *t = tile + fl * pitch + nl;
+            const float pm = t[0], pn = t[1], pp = t[2];
+            if (wd == 0.0f) {
+                v = wp * pn;
+            } else {
+                float D;
+                if (n == 0)            D = __fsub_rn(pp, pn);
+                else if (n == nt - 1)  D = __fsub_rn(pn, pm);
+                else                   D = 0.5f * __fsub_rn(pp, pm);
+                const float tn = __fadd_rn((float)n, t0fs);
+                v = wp * __fmaf_rn(-tn, D, pn);            // wp*(p - tn*D); wp = wd is 1 or 2 (exact)
+            }
+        }
+        out[idx] = v;
     }
 }
 
 }  // namespace
 
-int pat_launch_retile(const PatLaunchCtx &ctx, const float *src, float *tau_t, const int32_t *perm,
-                      int32_t nsens, int64_t npix, int64_t ntiles, int32_t sensor_begin, int32_t count) {
+int pat_launch_retile(const PatLaunchCtx &ctx, const float *src, float *u_t, const int32_t *perm,
+                      int32_t nsens, int64_t npix, int64_t ntiles, int32_t sensor_begin, int32_t count,
+                      float fs, float t0) {
     if (count <= 0 || ntiles <= 0) return 0;
     dim3 grid((unsigned)ntiles, (unsigned)(count < 64 ? count : 64));
-    retile_kernel<<<grid, kTilePix, 0, (cudaStream_t)ctx.stream>>>(src, tau_t, perm, nsens, npix,
-                                                                  sensor_begin, count);
+    retile_kernel<<<grid, kTilePix, 0, (cudaStream_t)ctx.stream>>>(src, u_t, perm, nsens, npix,
+                                                                  sensor_begin, count, fs, t0);
     return (int)cudaGetLastError();
 }
 
-int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *bd, float *images,
-                       int32_t nsens, int32_t nt, int32_t nframes, int64_t npix,
+int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, float *images,
+                       int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp, int64_t npix,
                        float wp, float wd, float t0fs) {
-    cudaStream_t st = (cudaStream_t)ctx.stream;
-    if (nframes == 1) {
-        const int64_t total = (int64_t)nsens * nt;
-        int64_t blocks = (total + 255) / 256;
-        const int64_t cap = (int64_t)ctx.num_sms * 8;
-        if (blocks > cap) blocks = cap;
-        if (blocks < 1) blocks = 1;
-        prepass_b1_kernel<<<(unsigned)blocks, 256, 0, st>>>(traces, (float2 *)bd, images, total, nt,
-                                                            npix, wp, wd, t0fs);
-    } else {
-        const int64_t row_elems = (int64_t)nt * nframes;
-        int64_t bx = (row_elems + 255) / 256;
-        int64_t cap = ((int64_t)ctx.num_sms * 8 + nsens - 1) / nsens;
-        if (cap < 1) cap = 1;
-        if (bx > cap) bx = cap;
-        dim3 grid((unsigned)bx, (unsigned)nsens);
-        prepass_batch_kernel<<<grid, 256, 0, st>>>(traces, (float2 *)bd, images, nsens, nt, nframes,
-                                                   npix, wp, wd, t0fs);
-    }
+    int log2_bp = 0;
+    while ((1 << log2_bp) < bp) ++log2_bp;
+    int32_t ns = 4096 / bp;                                // samples per block: bp*ns <= 4096 outputs
+    if (ns > 1024) ns = 1024;
+    if (ns > nt4) ns = nt4;
+    const int32_t groups = (nframes + bp - 1) / bp;
+    dim3 grid((unsigned)((nt4 + ns - 1) / ns), (unsigned)nsens, (unsigned)groups);
+    const size_t smem = (size_t)bp * (ns + 3) * sizeof(float);
+    prepass_kernel<<<grid, 256, smem, (cudaStream_t)ctx.stream>>>(traces, b, images, nsens, nt, nt4, nframes,
+                                                                log2_bp, ns, npix, wp, wd, t0fs);
     return (int)cudaGetLastError();
 }

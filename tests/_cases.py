@@ -50,7 +50,7 @@ def assert_parity(got, ref, what=""):
     return rel, mx / sc if sc > 0 else 0.0
 
 
-def gpu_backproject(geom, tau, traces, mode=1, max_batch=None, variant=0, host=False, t0=None):
+def gpu_backproject(geom, tau, traces, mode=1, max_batch=None, tuning=None, host=False, t0=None):
     """One pass of the product path through the C-ABI; returns fp32 images [B][P] (numpy)."""
     import torch
     import paper_1501_03869_b200 as pat
@@ -58,8 +58,8 @@ def gpu_backproject(geom, tau, traces, mode=1, max_batch=None, variant=0, host=F
     plan = pat.Plan(geom.n, geom.h, geom.origin, geom.c_map, geom.sensors, geom.roi_index, geom.nt,
                     geom.fs, geom.t0 if t0 is None else t0, weighting=mode, max_batch=max_batch or max(B, 1))
     try:
-        if variant:
-            pat.pat_set_gather_variant(plan.handle, variant)
+        if tuning:
+            pat.pat_set_gather_tuning(plan.handle, *tuning)
         plan.set_travel_times(tau)
         if host:
             tr = torch.from_numpy(np.ascontiguousarray(traces)).pin_memory()

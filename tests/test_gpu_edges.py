@@ -137,3 +137,55 @@ def test_compute_travel_times_on_plan_matches_host_fmm():
     torch.cuda.synchronize()
     assert_parity(img.cpu().numpy(), oracle.backproject(tau, tr, geom.fs), "plan-side FMM")
     plan.close()
+
+
+@pytest.mark.parametrize("B", [1, 2, 3, 4, 5, 8, 9, 16, 17, 32, 33, 64, 65, 130])
+def test_every_frame_count_class(B):
+    """Frame-count classes 1, 2, 3-4, ..., 33-64 and multi-group launches (> 64 frames)."""
+    g = _geom(700, 9, 160)
+    rng = np.random.default_rng(100 + B)
+    # smooth-ish tau (short windows, the fast path) with a few far outliers (segmented rows)
+    base = rng.uniform(20.0, 120.0, size=(9, 1))
+    tau = ((base + rng.uniform(0.0, 30.0, size=(9, 700))) / FS).astype(np.float32)
+    tau[2, ::50] = np.float32(3.0 / FS)
+    tr = rng.standard_normal((B, 9, 160)).astype(np.float32)
+    ref = oracle.backproject(tau, tr, FS, 0.0, 1)
+    assert_parity(gpu_backproject(g, tau, tr), ref, "B=%d" % B)
+
+
+@pytest.mark.parametrize("tuning", [(8, 1, 2), (16, 3, 2), (32, 5, 3), (64, 16, 4), (256, 2, 2), (128, 32, 2)])
+@pytest.mark.parametrize("B", [1, 4, 20])
+def test_gather_tuning_does_not_change_the_result(tuning, B):
+    """Window ring / slots / stages only change the schedule: segment splits, ring wrap-around,
+    null-padded chunks, pipeline depth."""
+    geom, tau = __import__("_cases").case(0)
+    tr = W.make_traces(geom, tau, frames=range(B))
+    ref = oracle.backproject(tau, tr, geom.fs, geom.t0, 1)
+    assert_parity(gpu_backproject(geom, tau, tr, tuning=tuning), ref, "tuning %s B=%d" % (tuning, B))
+    g = _geom(1500, 21, 300)
+    rng = np.random.default_rng(7)
+    tau2 = (rng.uniform(-5.0, 310.0, size=(21, 1500)) / FS).astype(np.float32)
+    tr2 = rng.standard_normal((B, 21, 300)).astype(np.float32)
+    assert_parity(gpu_backproject(g, tau2, tr2, tuning=tuning), oracle.backproject(tau2, tr2, FS, 0.0, 1),
+                  "random tau, tuning %s B=%d" % (tuning, B))
+
+
+def test_table_without_any_valid_entry_gives_zero_images():
+    g = _geom(300, 4, 64)
+    tau = np.full((4, 300), np.nan, np.float32)
+    tau[1] = -1.0
+    tau[2] = 1.0
+    tr = np.random.default_rng(8).standard_normal((3, 4, 64)).astype(np.float32)
+    got = gpu_backproject(g, tau, tr)
+    assert np.all(got == 0.0)
+
+
+def test_invalid_tuning_is_rejected():
+    import paper_1501_03869_b200 as pat
+    g = _geom(300, 4, 64)
+    plan = pat.Plan(g.n, g.h, g.origin, g.c_map, g.sensors, g.roi_index, g.nt, FS)
+    for bad in [(100, 0, 0), (4, 0, 0), (0, 33, 0), (0, 0, 1), (-8, 0, 0)]:
+        with pytest.raises(pat.PatError) as ei:
+            pat.pat_set_gather_tuning(plan.handle, *bad)
+        assert ei.value.status == pat.PAT_ERR_INVALID_ARG
+    plan.close()
