@@ -95,17 +95,22 @@ pat_status finalize_table(pat_plan *p, void *stream) {
     return PAT_OK;
 }
 
-struct Desc { int32_t tile, sensor, s0, w; };
+struct Entry { int32_t x, y, z, w; };       // one int4 of the work list (layout: gather.cu)
+struct Slot { int32_t row, sensor, s0, klen, len; bool whole; };
 
-// Work list for one shared-memory geometry: every row is cut into segments of at most wr-4
-// k-values (one descriptor each; rows without a valid pixel vanish), the descriptors are dealt
-// to grid_x persistent CTAs in equal shares and grouped into chunks of exactly R (null-padded);
-// a chunk never mixes tiles.  Bit 30 of w marks a chunk whose R descriptors are all whole rows.
+// Work list for one shared-memory geometry.  Every row with a valid pixel is cut into segments of
+// at most wr-4 k-values (one slot each; rows without a valid pixel vanish).  Slots are dealt to
+// grid_x persistent CTAs in equal shares and grouped into chunks of at most R slots that share a
+// tile and whose sample windows all lie inside one frame [cbase, cbase + wr) -- the window of a slot
+// is then ONE bulk copy to offset (s0 - cbase) and the consumers index it with k - cbase.
+// Chunk flags: simple = R whole rows (no per-slot range check needed); contig = the slots' u rows
+// are consecutive in the table (one bulk copy for the whole chunk).
 pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule **out) {
     const int64_t ntiles = p->dims.ntiles;
     const int32_t S = p->dims.nsens;
-    const int32_t step = cfg.wr - 4, R = cfg.R;
+    const int32_t step = cfg.wr - 4, R = cfg.R, wr = cfg.wr;
     const int32_t *meta = p->host_meta.data();
+    if ((int64_t)S * p->nt4 > (int64_t)INT32_MAX) return fail(p, PAT_ERR_UNSUPPORTED, "nsens*nt exceeds 2^31");
     int64_t V = 0;
     for (int64_t r = 0; r < ntiles * S; ++r) {
         const int32_t kmin = meta[2 * r], kmax = meta[2 * r + 1];
@@ -121,24 +126,30 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
     G = std::min<int64_t>(G, (V + R - 1) / R);
     sc.grid_x = (int)G;
     if (V == 0) { p->schedules.push_back(sc); *out = &p->schedules.back(); return PAT_OK; }
-    std::vector<Desc> list;
+    std::vector<Entry> list;
     std::vector<int32_t> cta_chunk;
+    const size_t per_chunk = (size_t)R + 1;
     try {
-        list.reserve((size_t)(V + (ntiles + G) * R));
+        list.reserve((size_t)(V / R + ntiles + G + 16) * per_chunk);
         cta_chunk.reserve((size_t)G + 1);
-        int64_t vi = 0, c = 0, vend = V / G;       // CTA c owns virtual rows [V*c/G, V*(c+1)/G)
-        size_t open = 0;                           // first descriptor of the open chunk
-        bool simple = true;
-        cta_chunk.push_back(0);
+        std::vector<Slot> cur;
+        int32_t cur_tile = -1, lo = 0, hi = 0;
         auto close_chunk = [&]() {
-            if (list.size() == open) return;
-            if (list.size() - open < (size_t)R) simple = false;
-            const int32_t tile = list[open].tile;
-            while (list.size() - open < (size_t)R) list.push_back(Desc{tile, 0, 0, 0});
-            if (simple) for (size_t q = open; q < list.size(); ++q) list[q].w |= 1 << 30;
-            open = list.size();
-            simple = true;
+            if (cur.empty()) return;
+            bool simple = (int32_t)cur.size() == R, contig = true;
+            for (size_t q = 0; q < cur.size(); ++q) {
+                simple = simple && cur[q].whole;
+                contig = contig && cur[q].row == cur[0].row + (int32_t)q;
+            }
+            const int32_t flags = (simple ? 1 : 0) | (contig ? 2 : 0) | ((int32_t)cur.size() << 8);
+            list.push_back(Entry{cur_tile, lo, flags, cur[0].row});
+            for (const Slot &sl : cur)
+                list.push_back(Entry{sl.row, sl.sensor * p->nt4 + sl.s0, (sl.s0 - lo) | (sl.len << 16), sl.klen});
+            for (int32_t q = (int32_t)cur.size(); q < R; ++q) list.push_back(Entry{0, 0, 0, 0});
+            cur.clear();
         };
+        int64_t vi = 0, c = 0, vend = V / G;       // CTA c owns slots [V*c/G, V*(c+1)/G)
+        cta_chunk.push_back(0);
         for (int64_t t = 0; t < ntiles; ++t) {
             for (int32_t s = 0; s < S; ++s) {
                 const int64_t r = t * S + s;
@@ -147,28 +158,45 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
                 const int32_t n0 = kmin & ~3, kend = kmax + 1;
                 const bool whole = kend - n0 <= step;
                 for (int32_t s0 = n0; s0 < kend; s0 += step) {
-                    if (vi == vend && c + 1 < G) {         // next CTA's share begins
+                    if (vi == vend && c + 1 < G) {         // the next CTA's share begins
                         close_chunk();
-                        cta_chunk.push_back((int32_t)(list.size() / R));
+                        cta_chunk.push_back((int32_t)(list.size() / per_chunk));
                         ++c;
                         vend = V * (c + 1) / G;
                     }
-                    if (list.size() > open && list[open].tile != (int32_t)t) close_chunk();
-                    list.push_back(Desc{(int32_t)t, s, s0, std::min(step, kend - s0)});
-                    if (!whole) simple = false;
-                    if (list.size() - open == (size_t)R) close_chunk();
+                    const int32_t klen = std::min(step, kend - s0);
+                    const int32_t len = (klen + 1 + 3) & ~3;               // samples s0 .. s0+klen
+                    if (!cur.empty() && (cur_tile != (int32_t)t || (int32_t)cur.size() == R ||
+                                         std::max(hi, s0 + len) - std::min(lo, s0) > wr))
+                        close_chunk();
+                    if (cur.empty()) { cur_tile = (int32_t)t; lo = s0; hi = s0 + len; }
+                    lo = std::min(lo, s0);
+                    hi = std::max(hi, s0 + len);
+                    cur.push_back(Slot{(int32_t)r, s, s0, klen, len, whole});
                     ++vi;
                 }
             }
         }
         close_chunk();
-        while ((int64_t)cta_chunk.size() < G + 1) cta_chunk.push_back((int32_t)(list.size() / R));
+        while ((int64_t)cta_chunk.size() < G + 1) cta_chunk.push_back((int32_t)(list.size() / per_chunk));
     } catch (...) { return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
-    if (list.size() / R > (size_t)INT32_MAX) return fail(p, PAT_ERR_UNSUPPORTED, "work list too long");
-    sc.nchunks = (int64_t)(list.size() / R);
-    cudaError_t ce = cudaMalloc(&sc.d_sched, list.size() * sizeof(Desc));
+    if (list.size() / per_chunk > (size_t)INT32_MAX) return fail(p, PAT_ERR_UNSUPPORTED, "work list too long");
+    sc.nchunks = (int64_t)(list.size() / per_chunk);
+    if (const char *dbg = std::getenv("PAT_DEBUG")) {
+        if (dbg[0] == '1') {
+            int64_t ns = 0, nc = 0, nreal = 0;
+            for (size_t q = 0; q < list.size(); q += per_chunk) {
+                ns += list[q].z & 1; nc += (list[q].z >> 1) & 1; nreal += list[q].z >> 8;
+            }
+            std::fprintf(stderr, "[pat] schedule bp=%d wr=%d R=%d stages=%d: grid=%d slots=%lld chunks=%lld "
+                         "(simple %lld, contig %lld, slots/chunk %.2f) smem=%zu B, %d CTA/SM\n", cfg.bp, cfg.wr, R,
+                         cfg.stages, sc.grid_x, (long long)V, (long long)sc.nchunks, (long long)ns, (long long)nc,
+                         (double)nreal / (double)sc.nchunks, pat_gather_smem_bytes(cfg), per_sm);
+        }
+    }
+    cudaError_t ce = cudaMalloc(&sc.d_sched, list.size() * sizeof(Entry));
     if (ce == cudaSuccess) ce = cudaMalloc((void **)&sc.d_cta_chunk, cta_chunk.size() * sizeof(int32_t));
-    if (ce == cudaSuccess) ce = cudaMemcpy(sc.d_sched, list.data(), list.size() * sizeof(Desc), cudaMemcpyHostToDevice);
+    if (ce == cudaSuccess) ce = cudaMemcpy(sc.d_sched, list.data(), list.size() * sizeof(Entry), cudaMemcpyHostToDevice);
     if (ce == cudaSuccess)
         ce = cudaMemcpy(sc.d_cta_chunk, cta_chunk.data(), cta_chunk.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
     if (ce != cudaSuccess) {
@@ -476,8 +504,8 @@ extern "C" int64_t pat_kernel_launches(const pat_plan *p) { return p ? p->launch
 
 extern "C" pat_status pat_set_gather_tuning(pat_plan *p, int32_t wr, int32_t rows, int32_t stages) {
     if (!p) return PAT_ERR_INVALID_ARG;
-    if (wr < 0 || rows < 0 || stages < 0 || rows > 32 || stages > 8 || (wr && (wr < 8 || wr > 4096 || (wr & (wr - 1)))))
-        return fail(p, PAT_ERR_INVALID_ARG, "wr: 0 or a power of two in [8, 4096]; rows: 0..32; stages: 0..8");
+    if (wr < 0 || rows < 0 || stages < 0 || rows > 31 || stages > 8 || (wr && (wr < 8 || wr > 4096 || (wr & (wr - 1)))))
+        return fail(p, PAT_ERR_INVALID_ARG, "wr: 0 or a power of two in [8, 4096]; rows: 0..31; stages: 0..8");
     if (stages == 1) return fail(p, PAT_ERR_INVALID_ARG, "stages must be 0 or >= 2");
     p->tune_wr = wr; p->tune_R = rows; p->tune_stages = stages;
     drop_schedules(p);
