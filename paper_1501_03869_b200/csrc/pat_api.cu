@@ -123,16 +123,17 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
     if (e) return cuda_fail(p, e, "gather occupancy query");
     if (per_sm < 1) return fail(p, PAT_ERR_CUDA, "gather kernel does not fit on an SM with this tuning");
     int64_t G = (int64_t)p->num_sms * per_sm;
-    G = std::min<int64_t>(G, (V + R - 1) / R);
-    sc.grid_x = (int)G;
+    sc.grid_x = 0;
     if (V == 0) { p->schedules.push_back(sc); *out = &p->schedules.back(); return PAT_OK; }
     std::vector<Entry> list;
     std::vector<int32_t> cta_chunk;
+    std::vector<int32_t> cost;                       // per chunk: fixed part + slots
+    int32_t chunk_cost = 6;
+    if (const char *cc = std::getenv("PAT_CHUNK_COST")) chunk_cost = std::max(0, std::atoi(cc));
     const size_t per_chunk = (size_t)R + 1;
     try {
-        list.reserve((size_t)(V / R + ntiles + G + 16) * per_chunk);
-        cta_chunk.reserve((size_t)G + 1);
-        std::vector<Slot> cur;
+        list.reserve((size_t)(V / R + ntiles + 16) * per_chunk);
+        std::vector<Slot> cur, rest;
         int32_t cur_tile = -1, lo = 0, hi = 0;
         auto close_chunk = [&]() {
             if (cur.empty()) return;
@@ -144,41 +145,62 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
             const int32_t flags = (simple ? 1 : 0) | (contig ? 2 : 0) | ((int32_t)cur.size() << 8);
             list.push_back(Entry{cur_tile, lo, flags, cur[0].row});
             for (const Slot &sl : cur)
-                list.push_back(Entry{sl.row, sl.sensor * p->nt4 + sl.s0, (sl.s0 - lo) | (sl.len << 16), sl.klen});
+                list.push_back(Entry{sl.row, sl.sensor * p->nt4 + sl.s0,
+                                     (int32_t)((uint32_t)(sl.s0 - lo) | ((uint32_t)sl.len << 16) | (contig ? 0x80000000u : 0u)),
+                                     sl.klen});
             for (int32_t q = (int32_t)cur.size(); q < R; ++q) list.push_back(Entry{0, 0, 0, 0});
+            cost.push_back(chunk_cost + (int32_t)cur.size());
             cur.clear();
         };
-        int64_t vi = 0, c = 0, vend = V / G;       // CTA c owns slots [V*c/G, V*(c+1)/G)
-        cta_chunk.push_back(0);
+        auto add_slot = [&](int32_t t, const Slot &sl) {
+            if (!cur.empty() && (cur_tile != t || (int32_t)cur.size() == R ||
+                                 std::max(hi, sl.s0 + sl.len) - std::min(lo, sl.s0) > wr))
+                close_chunk();
+            if (cur.empty()) { cur_tile = t; lo = sl.s0; hi = sl.s0 + sl.len; }
+            lo = std::min(lo, sl.s0);
+            hi = std::max(hi, sl.s0 + sl.len);
+            cur.push_back(sl);
+        };
         for (int64_t t = 0; t < ntiles; ++t) {
+            rest.clear();
+            // whole rows in sensor order (their u rows stay consecutive: one bulk copy per chunk) ...
             for (int32_t s = 0; s < S; ++s) {
                 const int64_t r = t * S + s;
                 const int32_t kmin = meta[2 * r], kmax = meta[2 * r + 1];
                 if (kmax < kmin) continue;
                 const int32_t n0 = kmin & ~3, kend = kmax + 1;
-                const bool whole = kend - n0 <= step;
-                for (int32_t s0 = n0; s0 < kend; s0 += step) {
-                    if (vi == vend && c + 1 < G) {         // the next CTA's share begins
-                        close_chunk();
-                        cta_chunk.push_back((int32_t)(list.size() / per_chunk));
-                        ++c;
-                        vend = V * (c + 1) / G;
+                if (kend - n0 <= step) {
+                    add_slot((int32_t)t, Slot{(int32_t)r, s, n0, kend - n0, (kend - n0 + 1 + 3) & ~3, true});
+                } else {
+                    for (int32_t s0 = n0; s0 < kend; s0 += step) {
+                        const int32_t klen = std::min(step, kend - s0);
+                        rest.push_back(Slot{(int32_t)r, s, s0, klen, (klen + 1 + 3) & ~3, false});
                     }
-                    const int32_t klen = std::min(step, kend - s0);
-                    const int32_t len = (klen + 1 + 3) & ~3;               // samples s0 .. s0+klen
-                    if (!cur.empty() && (cur_tile != (int32_t)t || (int32_t)cur.size() == R ||
-                                         std::max(hi, s0 + len) - std::min(lo, s0) > wr))
-                        close_chunk();
-                    if (cur.empty()) { cur_tile = (int32_t)t; lo = s0; hi = s0 + len; }
-                    lo = std::min(lo, s0);
-                    hi = std::max(hi, s0 + len);
-                    cur.push_back(Slot{(int32_t)r, s, s0, klen, len, whole});
-                    ++vi;
                 }
             }
+            // ... then the segments of the long rows, ordered in time so that they share frames
+            std::sort(rest.begin(), rest.end(), [](const Slot &a, const Slot &b) {
+                return a.s0 < b.s0 || (a.s0 == b.s0 && a.row < b.row);
+            });
+            for (const Slot &sl : rest) add_slot((int32_t)t, sl);
+            close_chunk();
         }
-        close_chunk();
-        while ((int64_t)cta_chunk.size() < G + 1) cta_chunk.push_back((int32_t)(list.size() / per_chunk));
+        // deal whole chunks to the CTAs in contiguous, equal-cost shares
+        const int64_t nchunks = (int64_t)cost.size();
+        G = std::min<int64_t>(G, nchunks);
+        sc.grid_x = (int)G;
+        int64_t total = 0;
+        for (int32_t cc : cost) total += cc;
+        cta_chunk.reserve((size_t)G + 1);
+        cta_chunk.push_back(0);
+        int64_t q = 0, acc = 0;                     // acc = cost of chunks [0, q)
+        for (int64_t c = 1; c < G; ++c) {
+            const int64_t want = total * c / G;
+            const int64_t qmin = cta_chunk.back() + 1, qmax = nchunks - (G - c);
+            while (q < qmax && (q < qmin || acc + cost[q] / 2 < want)) acc += cost[q++];
+            cta_chunk.push_back((int32_t)q);
+        }
+        cta_chunk.push_back((int32_t)nchunks);
     } catch (...) { return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
     if (list.size() / per_chunk > (size_t)INT32_MAX) return fail(p, PAT_ERR_UNSUPPORTED, "work list too long");
     sc.nchunks = (int64_t)(list.size() / per_chunk);
