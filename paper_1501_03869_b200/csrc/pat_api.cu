@@ -96,7 +96,7 @@ pat_status finalize_table(pat_plan *p, void *stream) {
 }
 
 struct Entry { int32_t x, y, z, w; };       // one int4 of the work list (layout: gather.cu)
-struct Slot { int32_t row, sensor, s0, klen, len; bool whole; };
+struct Slot { int32_t row, sensor, s0, klen, len; bool whole, allvalid; };
 
 // Work list for one shared-memory geometry.  Every row with a valid pixel is cut into segments of
 // at most wr-4 k-values (one slot each; rows without a valid pixel vanish).  Slots are dealt to
@@ -113,7 +113,7 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
     if ((int64_t)S * p->nt4 > (int64_t)INT32_MAX) return fail(p, PAT_ERR_UNSUPPORTED, "nsens*nt exceeds 2^31");
     int64_t V = 0;
     for (int64_t r = 0; r < ntiles * S; ++r) {
-        const int32_t kmin = meta[2 * r], kmax = meta[2 * r + 1];
+        const int32_t kmin = meta[2 * r], kmax = meta[2 * r + 1] < 0 ? -1 : (meta[2 * r + 1] & 0x3FFFFFFF);
         if (kmax >= kmin) V += (kmax + 1 - (kmin & ~3) + step - 1) / step;
     }
     PatSchedule sc;
@@ -137,12 +137,13 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
         int32_t cur_tile = -1, lo = 0, hi = 0;
         auto close_chunk = [&]() {
             if (cur.empty()) return;
-            bool simple = (int32_t)cur.size() == R, contig = true;
+            bool simple = (int32_t)cur.size() == R, contig = true, allvalid = true;
             for (size_t q = 0; q < cur.size(); ++q) {
                 simple = simple && cur[q].whole;
+                allvalid = allvalid && cur[q].allvalid;
                 contig = contig && cur[q].row == cur[0].row + (int32_t)q;
             }
-            const int32_t flags = (simple ? 1 : 0) | (contig ? 2 : 0) | ((int32_t)cur.size() << 8);
+            const int32_t flags = (simple ? 1 : 0) | (contig ? 2 : 0) | (allvalid ? 4 : 0) | ((int32_t)cur.size() << 8);
             list.push_back(Entry{cur_tile, lo, flags, cur[0].row});
             for (const Slot &sl : cur)
                 list.push_back(Entry{sl.row, sl.sensor * p->nt4 + sl.s0,
@@ -166,15 +167,16 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
             // whole rows in sensor order (their u rows stay consecutive: one bulk copy per chunk) ...
             for (int32_t s = 0; s < S; ++s) {
                 const int64_t r = t * S + s;
-                const int32_t kmin = meta[2 * r], kmax = meta[2 * r + 1];
+                const int32_t kmin = meta[2 * r], kmax = meta[2 * r + 1] < 0 ? -1 : (meta[2 * r + 1] & 0x3FFFFFFF);
                 if (kmax < kmin) continue;
+                const bool allvalid = (meta[2 * r + 1] >> 30) & 1;
                 const int32_t n0 = kmin & ~3, kend = kmax + 1;
                 if (kend - n0 <= step) {
-                    add_slot((int32_t)t, Slot{(int32_t)r, s, n0, kend - n0, (kend - n0 + 1 + 3) & ~3, true});
+                    add_slot((int32_t)t, Slot{(int32_t)r, s, n0, kend - n0, (kend - n0 + 1 + 3) & ~3, true, allvalid});
                 } else {
                     for (int32_t s0 = n0; s0 < kend; s0 += step) {
                         const int32_t klen = std::min(step, kend - s0);
-                        rest.push_back(Slot{(int32_t)r, s, s0, klen, (klen + 1 + 3) & ~3, false});
+                        rest.push_back(Slot{(int32_t)r, s, s0, klen, (klen + 1 + 3) & ~3, false, false});
                     }
                 }
             }
@@ -248,7 +250,7 @@ PatLayout pat_layout(const PatDims &d) {
     L.meta = take((size_t)d.ntiles * d.nsens * 2 * sizeof(int32_t));
     const int bp = pat_frames_per_group(d.max_batch);
     const size_t padded = (size_t)(d.max_batch + bp - 1) / bp * bp;
-    L.bd = take(padded * d.nsens * ((d.nt + 3) / 4 * 4) * sizeof(float));
+    L.bd = take(std::max<size_t>(padded, 4) * d.nsens * ((d.nt + 3) / 4 * 4) * sizeof(float));
     L.perm = take((size_t)d.ntiles * kTilePix * sizeof(int32_t));
     L.traces = take((size_t)d.max_batch * d.nsens * d.nt * sizeof(float));
     L.images = take((size_t)d.max_batch * d.npix * sizeof(float));
@@ -460,7 +462,8 @@ extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *i
     }
     float *bw = (float *)(p->ws + p->lay.bd);
     const float t0fs = (float)((double)p->t0 * (double)p->fs);
-    int e = pat_launch_prepass(ctx, d_tr, bw, d_img, d.nsens, d.nt, p->nt4, nframes, bp, d.npix, p->wp, p->wd, t0fs);
+    int e = pat_launch_prepass(ctx, d_tr, bw, d_img, d.nsens, d.nt, p->nt4, nframes, bp,
+                               pat_gather_elem_floats(bp) == 2, d.npix, p->wp, p->wd, t0fs);
     if (e) return cuda_fail(p, e, "pre-pass launch");
     ++p->launches;
     if (prof) cudaEventRecord(ev[1], st);

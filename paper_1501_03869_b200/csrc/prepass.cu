@@ -27,8 +27,22 @@ retile_kernel(const float *__restrict__ src, float *__restrict__ u_t,
 }
 
 // ---- H1 -----------------------------------------------------------------------------------
+// b[n] from the staged samples p[n-1], p[n], p[n+1] (t points at p[n-1]).
+__device__ __forceinline__ float weight_at(const float *t, int32_t n, int32_t nt, float wp, float wd, float t0fs) {
+    const float pm = t[0], pn = t[1], pp = t[2];
+    if (wd == 0.0f) return wp * pn;
+    float D;
+    if (n == 0)            D = __fsub_rn(pp, pn);
+    else if (n == nt - 1)  D = __fsub_rn(pn, pm);
+    else                   D = 0.5f * __fsub_rn(pp, pm);
+    const float tn = __fadd_rn((float)n, t0fs);
+    return wp * __fmaf_rn(-tn, D, pn);                     // wp*(p - tn*D); wp = wd is 1 or 2 (exact)
+}
+
 // Block = (sample chunk, sensor, frame group).  The chunk of every frame of the group is read
-// coalesced along time into shared memory (+1 halo each side), then written frame-fastest.
+// coalesced along time into shared memory (halo -1 / +2), then written frame-fastest; PAIRS writes
+// {b[n], b[n+1]-b[n]} (the gather's one-load interpolation operand for Bp <= 2).
+template <bool PAIRS>
 __global__ void __launch_bounds__(256)
 prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
                int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t log2_bp, int32_t ns,
@@ -48,33 +62,25 @@ prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *_
     for (int32_t fl = warp; fl < bp; fl += 8) {
         const int32_t f = grp * bp + fl;
         const float *p = traces + ((int64_t)f * nsens + s) * nt;
-        for (int32_t j = lane; j < ns + 2; j += 32) {
+        for (int32_t j = lane; j < ns + 3; j += 32) {
             const int32_t n = n_begin - 1 + j;
             tile[fl * pitch + j] = (f < nframes && n >= 0 && n < nt) ? __ldg(p + n) : 0.0f;
         }
     }
     __syncthreads();
-    float *out = b + (((int64_t)grp * nsens + s) * nt4 + n_begin) * bp;
+    const int64_t obase = (((int64_t)grp * nsens + s) * nt4 + n_begin) * bp;
     const int32_t nloc = min(ns, nt4 - n_begin);
     for (int32_t idx = threadIdx.x; idx < (nloc << log2_bp); idx += 256) {
         const int32_t nl = idx >> log2_bp, fl = idx & (bp - 1);
         const int32_t n = n_begin + nl;
-        float v = 0.0f;
+        float v = 0.0f, d = 0.0f;
         if (n < nt && grp * bp + fl < nframes) {
             const float *t = tile + fl * pitch + nl;
-            const float pm = t[0], pn = t[1], pp = t[2];
-            if (wd == 0.0f) {
-                v = wp * pn;
-            } else {
-                float D;
-                if (n == 0)            D = __fsub_rn(pp, pn);
-                else if (n == nt - 1)  D = __fsub_rn(pn, pm);
-                else                   D = 0.5f * __fsub_rn(pp, pm);
-                const float tn = __fadd_rn((float)n, t0fs);
-                v = wp * __fmaf_rn(-tn, D, pn);            // wp*(p - tn*D); wp = wd is 1 or 2 (exact)
-            }
+            v = weight_at(t, n, nt, wp, wd, t0fs);
+            if (PAIRS && n + 1 < nt) d = __fsub_rn(weight_at(t + 1, n + 1, nt, wp, wd, t0fs), v);
         }
-        out[idx] = v;
+        if (PAIRS) reinterpret_cast<float2 *>(b)[obase + idx] = make_float2(v, d);
+        else b[obase + idx] = v;
     }
 }
 
@@ -91,8 +97,8 @@ int pat_launch_retile(const PatLaunchCtx &ctx, const float *src, float *u_t, con
 }
 
 int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, float *images,
-                       int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp, int64_t npix,
-                       float wp, float wd, float t0fs) {
+                       int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp, bool pairs,
+                       int64_t npix, float wp, float wd, float t0fs) {
     int log2_bp = 0;
     while ((1 << log2_bp) < bp) ++log2_bp;
     int32_t ns = 4096 / bp;                                // samples per block: bp*ns <= 4096 outputs
@@ -101,7 +107,11 @@ int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, f
     const int32_t groups = (nframes + bp - 1) / bp;
     dim3 grid((unsigned)((nt4 + ns - 1) / ns), (unsigned)nsens, (unsigned)groups);
     const size_t smem = (size_t)bp * (ns + 3) * sizeof(float);
-    prepass_kernel<<<grid, 256, smem, (cudaStream_t)ctx.stream>>>(traces, b, images, nsens, nt, nt4, nframes,
-                                                                log2_bp, ns, npix, wp, wd, t0fs);
+    if (pairs)
+        prepass_kernel<true><<<grid, 256, smem, (cudaStream_t)ctx.stream>>>(traces, b, images, nsens, nt, nt4,
+                                                                          nframes, log2_bp, ns, npix, wp, wd, t0fs);
+    else
+        prepass_kernel<false><<<grid, 256, smem, (cudaStream_t)ctx.stream>>>(traces, b, images, nsens, nt, nt4,
+                                                                           nframes, log2_bp, ns, npix, wp, wd, t0fs);
     return (int)cudaGetLastError();
 }
