@@ -124,13 +124,13 @@ const char *pat_last_error(const pat_plan *plan);
 int64_t pat_kernel_launches(const pat_plan *plan);
 
 /* Override the gather's shared-memory geometry (tuning / test hook; 0 = choose automatically):
- *   wr      window ring in samples, a power of two in [8, 4096]: a (tile, sensor) row whose pixels
- *           span more than wr-4 samples of the trace is processed in several segments, and the rows
- *           of one pipeline stage must fit a common wr-sample frame;
- *   rows    (tile, sensor) rows per pipeline stage, 1..31;   stages  pipeline depth, 2..8.
+ *   wr      longest trace window one (tile, sensor) row may occupy in shared memory, a power of two in
+ *           [8, 4096] (clipped to the frame-count class's limit): a row whose pixels span more than
+ *           wr-4 samples is processed in several segments;
+ *   rows    (tile, sensor) rows per pipeline stage, 1..30;   stages  pipeline depth, 2..8.
  * A request that does not fit one CTA's shared memory for a given frame-count class is shrunk
- * (rows, then stages, then wr).  Takes effect at the next pat_backproject (the work lists are
- * rebuilt).  Results do not depend on the tuning beyond fp32 summation order. */
+ * (rows, then stages).  Takes effect at the next pat_backproject (the work lists are rebuilt).
+ * Results do not depend on the tuning beyond fp32 summation order. */
 pat_status pat_set_gather_tuning(pat_plan *plan, int32_t wr, int32_t rows, int32_t stages);
 
 /* Measurement helper (bench.py's roofline leg): while enabled, pat_backproject brackets the

@@ -108,7 +108,7 @@ struct Slot { int32_t row, sensor, s0, klen, len; bool whole, allvalid; };
 pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule **out) {
     const int64_t ntiles = p->dims.ntiles;
     const int32_t S = p->dims.nsens;
-    const int32_t step = cfg.wr - 4, R = cfg.R, wr = cfg.wr;
+    const int32_t step = cfg.wr - 4, R = cfg.R;
     const int32_t *meta = p->host_meta.data();
     if ((int64_t)S * p->nt4 > (int64_t)INT32_MAX) return fail(p, PAT_ERR_UNSUPPORTED, "nsens*nt exceeds 2^31");
     int64_t V = 0;
@@ -134,32 +134,32 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
     try {
         list.reserve((size_t)(V / R + ntiles + 16) * per_chunk);
         std::vector<Slot> cur, rest;
-        int32_t cur_tile = -1, lo = 0, hi = 0;
+        int32_t cur_tile = -1, used = 0;             // used = window samples already packed into the chunk
         auto close_chunk = [&]() {
             if (cur.empty()) return;
-            bool simple = (int32_t)cur.size() == R, contig = true, allvalid = true;
+            bool fast = (int32_t)cur.size() == R, contig = true;
             for (size_t q = 0; q < cur.size(); ++q) {
-                simple = simple && cur[q].whole;
-                allvalid = allvalid && cur[q].allvalid;
+                fast = fast && cur[q].whole && cur[q].allvalid;
                 contig = contig && cur[q].row == cur[0].row + (int32_t)q;
             }
-            const int32_t flags = (simple ? 1 : 0) | (contig ? 2 : 0) | (allvalid ? 4 : 0) | ((int32_t)cur.size() << 8);
-            list.push_back(Entry{cur_tile, lo, flags, cur[0].row});
-            for (const Slot &sl : cur)
+            const int32_t flags = (fast ? 1 : 0) | (contig ? 2 : 0) | ((int32_t)cur.size() << 8);
+            list.push_back(Entry{cur_tile, 0, flags, cur[0].row});
+            int32_t pos = 0;
+            for (const Slot &sl : cur) {
                 list.push_back(Entry{sl.row, sl.sensor * p->nt4 + sl.s0,
-                                     (int32_t)((uint32_t)(sl.s0 - lo) | ((uint32_t)sl.len << 16) | (contig ? 0x80000000u : 0u)),
-                                     sl.klen});
+                                     (int32_t)((uint32_t)pos | ((uint32_t)sl.klen << 16) | (contig ? 0x80000000u : 0u)),
+                                     sl.s0});
+                pos += sl.len;
+            }
             for (int32_t q = (int32_t)cur.size(); q < R; ++q) list.push_back(Entry{0, 0, 0, 0});
-            cost.push_back(chunk_cost + (int32_t)cur.size());
+            cost.push_back(chunk_cost + (int32_t)cur.size() * (fast ? 2 : 3));
             cur.clear();
+            used = 0;
         };
         auto add_slot = [&](int32_t t, const Slot &sl) {
-            if (!cur.empty() && (cur_tile != t || (int32_t)cur.size() == R ||
-                                 std::max(hi, sl.s0 + sl.len) - std::min(lo, sl.s0) > wr))
-                close_chunk();
-            if (cur.empty()) { cur_tile = t; lo = sl.s0; hi = sl.s0 + sl.len; }
-            lo = std::min(lo, sl.s0);
-            hi = std::max(hi, sl.s0 + sl.len);
+            if (!cur.empty() && (cur_tile != t || (int32_t)cur.size() == R || used + sl.len > cfg.cap)) close_chunk();
+            cur_tile = t;
+            used += sl.len;
             cur.push_back(sl);
         };
         for (int64_t t = 0; t < ntiles; ++t) {
@@ -172,18 +172,15 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
                 const bool allvalid = (meta[2 * r + 1] >> 30) & 1;
                 const int32_t n0 = kmin & ~3, kend = kmax + 1;
                 if (kend - n0 <= step) {
-                    add_slot((int32_t)t, Slot{(int32_t)r, s, n0, kend - n0, (kend - n0 + 1 + 3) & ~3, true, allvalid});
+                    add_slot((int32_t)t, Slot{(int32_t)r, s, n0, kend - n0, (kend - n0 + 4) & ~3, true, allvalid});
                 } else {
                     for (int32_t s0 = n0; s0 < kend; s0 += step) {
                         const int32_t klen = std::min(step, kend - s0);
-                        rest.push_back(Slot{(int32_t)r, s, s0, klen, (klen + 1 + 3) & ~3, false, false});
+                        rest.push_back(Slot{(int32_t)r, s, s0, klen, (klen + 4) & ~3, false, false});
                     }
                 }
             }
-            // ... then the segments of the long rows, ordered in time so that they share frames
-            std::sort(rest.begin(), rest.end(), [](const Slot &a, const Slot &b) {
-                return a.s0 < b.s0 || (a.s0 == b.s0 && a.row < b.row);
-            });
+            // ... then the segments of the long rows
             for (const Slot &sl : rest) add_slot((int32_t)t, sl);
             close_chunk();
         }
@@ -213,7 +210,7 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
                 ns += list[q].z & 1; nc += (list[q].z >> 1) & 1; nreal += list[q].z >> 8;
             }
             std::fprintf(stderr, "[pat] schedule bp=%d wr=%d R=%d stages=%d: grid=%d slots=%lld chunks=%lld "
-                         "(simple %lld, contig %lld, slots/chunk %.2f) smem=%zu B, %d CTA/SM\n", cfg.bp, cfg.wr, R,
+                         "(fast %lld, contig %lld, slots/chunk %.2f) smem=%zu B, %d CTA/SM\n", cfg.bp, cfg.wr, R,
                          cfg.stages, sc.grid_x, (long long)V, (long long)sc.nchunks, (long long)ns, (long long)nc,
                          (double)nreal / (double)sc.nchunks, pat_gather_smem_bytes(cfg), per_sm);
         }
@@ -250,7 +247,7 @@ PatLayout pat_layout(const PatDims &d) {
     L.meta = take((size_t)d.ntiles * d.nsens * 2 * sizeof(int32_t));
     const int bp = pat_frames_per_group(d.max_batch);
     const size_t padded = (size_t)(d.max_batch + bp - 1) / bp * bp;
-    L.bd = take(std::max<size_t>(padded, 4) * d.nsens * ((d.nt + 3) / 4 * 4) * sizeof(float));
+    L.bd = take(padded * d.nsens * ((d.nt + 3) / 4 * 4) * sizeof(float));
     L.perm = take((size_t)d.ntiles * kTilePix * sizeof(int32_t));
     L.traces = take((size_t)d.max_batch * d.nsens * d.nt * sizeof(float));
     L.images = take((size_t)d.max_batch * d.npix * sizeof(float));
@@ -462,8 +459,7 @@ extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *i
     }
     float *bw = (float *)(p->ws + p->lay.bd);
     const float t0fs = (float)((double)p->t0 * (double)p->fs);
-    int e = pat_launch_prepass(ctx, d_tr, bw, d_img, d.nsens, d.nt, p->nt4, nframes, bp,
-                               pat_gather_elem_floats(bp) == 2, d.npix, p->wp, p->wd, t0fs);
+    int e = pat_launch_prepass(ctx, d_tr, bw, d_img, d.nsens, d.nt, p->nt4, nframes, bp, d.npix, p->wp, p->wd, t0fs);
     if (e) return cuda_fail(p, e, "pre-pass launch");
     ++p->launches;
     if (prof) cudaEventRecord(ev[1], st);
@@ -529,8 +525,8 @@ extern "C" int64_t pat_kernel_launches(const pat_plan *p) { return p ? p->launch
 
 extern "C" pat_status pat_set_gather_tuning(pat_plan *p, int32_t wr, int32_t rows, int32_t stages) {
     if (!p) return PAT_ERR_INVALID_ARG;
-    if (wr < 0 || rows < 0 || stages < 0 || rows > 31 || stages > 8 || (wr && (wr < 8 || wr > 4096 || (wr & (wr - 1)))))
-        return fail(p, PAT_ERR_INVALID_ARG, "wr: 0 or a power of two in [8, 4096]; rows: 0..31; stages: 0..8");
+    if (wr < 0 || rows < 0 || stages < 0 || rows > 30 || stages > 8 || (wr && (wr < 8 || wr > 4096 || (wr & (wr - 1)))))
+        return fail(p, PAT_ERR_INVALID_ARG, "wr: 0 or a power of two in [8, 4096]; rows: 0..30; stages: 0..8");
     if (stages == 1) return fail(p, PAT_ERR_INVALID_ARG, "stages must be 0 or >= 2");
     p->tune_wr = wr; p->tune_R = rows; p->tune_stages = stages;
     drop_schedules(p);

@@ -40,9 +40,7 @@ __device__ __forceinline__ float weight_at(const float *t, int32_t n, int32_t nt
 }
 
 // Block = (sample chunk, sensor, frame group).  The chunk of every frame of the group is read
-// coalesced along time into shared memory (halo -1 / +2), then written frame-fastest; PAIRS writes
-// {b[n], b[n+1]-b[n]} (the gather's one-load interpolation operand for Bp <= 2).
-template <bool PAIRS>
+// coalesced along time into shared memory (+1 halo each side), then written frame-fastest.
 __global__ void __launch_bounds__(256)
 prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
                int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t log2_bp, int32_t ns,
@@ -62,7 +60,7 @@ prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *_
     for (int32_t fl = warp; fl < bp; fl += 8) {
         const int32_t f = grp * bp + fl;
         const float *p = traces + ((int64_t)f * nsens + s) * nt;
-        for (int32_t j = lane; j < ns + 3; j += 32) {
+        for (int32_t j = lane; j < ns + 2; j += 32) {
             const int32_t n = n_begin - 1 + j;
             tile[fl * pitch + j] = (f < nframes && n >= 0 && n < nt) ? __ldg(p + n) : 0.0f;
         }
@@ -73,14 +71,9 @@ prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *_
     for (int32_t idx = threadIdx.x; idx < (nloc << log2_bp); idx += 256) {
         const int32_t nl = idx >> log2_bp, fl = idx & (bp - 1);
         const int32_t n = n_begin + nl;
-        float v = 0.0f, d = 0.0f;
-        if (n < nt && grp * bp + fl < nframes) {
-            const float *t = tile + fl * pitch + nl;
-            v = weight_at(t, n, nt, wp, wd, t0fs);
-            if (PAIRS && n + 1 < nt) d = __fsub_rn(weight_at(t + 1, n + 1, nt, wp, wd, t0fs), v);
-        }
-        if (PAIRS) reinterpret_cast<float2 *>(b)[obase + idx] = make_float2(v, d);
-        else b[obase + idx] = v;
+        float v = 0.0f;
+        if (n < nt && grp * bp + fl < nframes) v = weight_at(tile + fl * pitch + nl, n, nt, wp, wd, t0fs);
+        b[obase + idx] = v;
     }
 }
 
@@ -97,7 +90,7 @@ int pat_launch_retile(const PatLaunchCtx &ctx, const float *src, float *u_t, con
 }
 
 int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, float *images,
-                       int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp, bool pairs,
+                       int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp,
                        int64_t npix, float wp, float wd, float t0fs) {
     int log2_bp = 0;
     while ((1 << log2_bp) < bp) ++log2_bp;
@@ -107,11 +100,7 @@ int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, f
     const int32_t groups = (nframes + bp - 1) / bp;
     dim3 grid((unsigned)((nt4 + ns - 1) / ns), (unsigned)nsens, (unsigned)groups);
     const size_t smem = (size_t)bp * (ns + 3) * sizeof(float);
-    if (pairs)
-        prepass_kernel<true><<<grid, 256, smem, (cudaStream_t)ctx.stream>>>(traces, b, images, nsens, nt, nt4,
-                                                                          nframes, log2_bp, ns, npix, wp, wd, t0fs);
-    else
-        prepass_kernel<false><<<grid, 256, smem, (cudaStream_t)ctx.stream>>>(traces, b, images, nsens, nt, nt4,
-                                                                           nframes, log2_bp, ns, npix, wp, wd, t0fs);
+    prepass_kernel<<<grid, 256, smem, (cudaStream_t)ctx.stream>>>(traces, b, images, nsens, nt, nt4, nframes,
+                                                                log2_bp, ns, npix, wp, wd, t0fs);
     return (int)cudaGetLastError();
 }
