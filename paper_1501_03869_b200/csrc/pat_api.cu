@@ -137,7 +137,7 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
         int32_t cur_tile = -1, used = 0;             // used = window samples already packed into the chunk
         auto close_chunk = [&]() {
             if (cur.empty()) return;
-            bool fast = (int32_t)cur.size() == R, contig = true;
+            bool fast = true, contig = true;
             for (size_t q = 0; q < cur.size(); ++q) {
                 fast = fast && cur[q].whole && cur[q].allvalid;
                 contig = contig && cur[q].row == cur[0].row + (int32_t)q;

@@ -57,10 +57,13 @@ prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *_
         for (int64_t q = blk * 256 + threadIdx.x; q < tot; q += nblk * 256) images[q] = 0.0f;
     }
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int32_t fl = warp; fl < bp; fl += 8) {
+    // long rows: the whole block strides one frame's row; short rows: one warp per frame
+    const int32_t nw = ns + 2 >= 256 ? 1 : 8, wid = ns + 2 >= 256 ? 0 : warp;
+    const int32_t lid = ns + 2 >= 256 ? (int32_t)threadIdx.x : lane, lstep = ns + 2 >= 256 ? 256 : 32;
+    for (int32_t fl = wid; fl < bp; fl += nw) {
         const int32_t f = grp * bp + fl;
         const float *p = traces + ((int64_t)f * nsens + s) * nt;
-        for (int32_t j = lane; j < ns + 2; j += 32) {
+        for (int32_t j = lid; j < ns + 2; j += lstep) {
             const int32_t n = n_begin - 1 + j;
             tile[fl * pitch + j] = (f < nframes && n >= 0 && n < nt) ? __ldg(p + n) : 0.0f;
         }
@@ -74,6 +77,32 @@ prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *_
         float v = 0.0f;
         if (n < nt && grp * bp + fl < nframes) v = weight_at(tile + fl * pitch + nl, n, nt, wp, wd, t0fs);
         b[obase + idx] = v;
+    }
+}
+
+// Bp = 1: no transposition needed -- one thread per 4 consecutive samples, straight from global
+// memory (the +-1 neighbours come from L1), 16-byte stores.
+__global__ void __launch_bounds__(256)
+prepass_b1_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
+                  int32_t nsens, int32_t nt, int32_t nt4, int64_t npix, float wp, float wd, float t0fs) {
+    asm volatile("griddepcontrol.launch_dependents;");
+    const int64_t gid = (int64_t)blockIdx.x * 256 + threadIdx.x, nthr = (int64_t)gridDim.x * 256;
+    for (int64_t q = gid; q < npix; q += nthr) images[q] = 0.0f;
+    const int32_t quads = nt4 >> 2;
+    for (int64_t q = gid; q < (int64_t)nsens * quads; q += nthr) {
+        const int32_t s = (int32_t)(q / quads), n0 = (int32_t)(q - (int64_t)s * quads) << 2;
+        const float *p = traces + (int64_t)s * nt;
+        float w[6];                                        // p[n0-1 .. n0+4]
+#pragma unroll
+        for (int j = 0; j < 6; ++j) {
+            const int32_t n = n0 - 1 + j;
+            w[j] = (n >= 0 && n < nt) ? __ldg(p + n) : 0.0f;
+        }
+        float4 o;
+        float *ov = reinterpret_cast<float *>(&o);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) ov[j] = (n0 + j < nt) ? weight_at(w + j, n0 + j, nt, wp, wd, t0fs) : 0.0f;
+        *reinterpret_cast<float4 *>(b + (int64_t)s * nt4 + n0) = o;
     }
 }
 
@@ -92,6 +121,14 @@ int pat_launch_retile(const PatLaunchCtx &ctx, const float *src, float *u_t, con
 int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, float *images,
                        int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp,
                        int64_t npix, float wp, float wd, float t0fs) {
+    if (bp == 1) {
+        const int64_t work = (int64_t)nsens * (nt4 >> 2);
+        int64_t blocks = (work + 255) / 256;
+        if (blocks > (int64_t)ctx.num_sms * 16) blocks = (int64_t)ctx.num_sms * 16;
+        prepass_b1_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)ctx.stream>>>(traces, b, images, nsens, nt, nt4,
+                                                                                  npix, wp, wd, t0fs);
+        return (int)cudaGetLastError();
+    }
     int log2_bp = 0;
     while ((1 << log2_bp) < bp) ++log2_bp;
     int32_t ns = 4096 / bp;                                // samples per block: bp*ns <= 4096 outputs
