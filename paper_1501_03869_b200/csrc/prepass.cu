@@ -57,13 +57,10 @@ prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *_
         for (int64_t q = blk * 256 + threadIdx.x; q < tot; q += nblk * 256) images[q] = 0.0f;
     }
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    // long rows: the whole block strides one frame's row; short rows: one warp per frame
-    const int32_t nw = ns + 2 >= 256 ? 1 : 8, wid = ns + 2 >= 256 ? 0 : warp;
-    const int32_t lid = ns + 2 >= 256 ? (int32_t)threadIdx.x : lane, lstep = ns + 2 >= 256 ? 256 : 32;
-    for (int32_t fl = wid; fl < bp; fl += nw) {
+    for (int32_t fl = warp; fl < bp; fl += 8) {
         const int32_t f = grp * bp + fl;
         const float *p = traces + ((int64_t)f * nsens + s) * nt;
-        for (int32_t j = lid; j < ns + 2; j += lstep) {
+        for (int32_t j = lane; j < ns + 2; j += 32) {
             const int32_t n = n_begin - 1 + j;
             tile[fl * pitch + j] = (f < nframes && n >= 0 && n < nt) ? __ldg(p + n) : 0.0f;
         }
