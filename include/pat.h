@@ -103,7 +103,7 @@ pat_status pat_set_travel_times(pat_plan *plan, const float *tau, int32_t sensor
  * Both DEVICE (16-byte aligned) or both HOST pointers (detected; host buffers should be
  * pinned for the copies to be asynchronous).  Enqueues weighting pre-pass + gather (+ the
  * copies for host buffers) on `stream` and returns without synchronising -- except for the first
- * call with a given frame-count class (1, 2, 3-4, 5-8, ..., 33+) after the table changed, which
+ * call with a given frame-count class (1, 2, 3-4, 5-8, 9-16, 17+) after the table changed, which
  * builds that class's work list (a few hundred KB of library-owned device memory, freed by
  * pat_destroy) and must therefore not happen inside a stream capture.
  * nframes = 0 is a no-op; nframes > max_batch -> PAT_ERR_INVALID_ARG; tau rows missing ->
