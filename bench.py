@@ -12,8 +12,9 @@ CPU FMM (input preparation, untimed).  Prints ONE JSON line (rank 0):
                that holds one step on each of R rotating plans (R * tau bytes > 3 x L2, so the tau
                stream cannot be served from L2).
   roofline     the gather kernel alone: algorithmic bytes per launch (tau + traces + images,
-               north_star's definition) / its mean duration from CUDA events inside the library
-               (pat_set_profiling), against the measured HBM copy peak of MEASURED_PEAKS.json.
+               north_star's definition) / its mean launch duration (the gather launched back to back
+               from the same kind of CUDA graph, pat_set_profiling mode 2, CUDA events around the
+               region), against the measured HBM copy peak of MEASURED_PEAKS.json.
   e2e          the same metric through the C-ABI with pinned HOST traces/images (H2D + D2H timed).
   cpu_baseline the oracle (oracle/pat_oracle.c) timed on this box's host cores, rank 0, N = 1.
   sweep        B = 1..64 on the same geometry (N = 1 only): ms/frame, GUpd/s, HBM fraction and the
@@ -239,22 +240,20 @@ def time_steps(rig, nsteps, warmup, dist=None):
     return ms
 
 
-def profile_gather(rig, nsteps):
-    """Mean device duration (ms) of the pre-pass and of the gather kernel over nsteps direct calls,
-    from CUDA events recorded by the library on the launching stream."""
+def kernel_only_ms(rig, mode, nsteps, warmup):
+    """Mean device duration (ms per launch) of ONE kernel of the step -- mode 2 = the gather, 3 = the
+    pre-pass (pat_set_profiling) -- launched back to back from a CUDA graph over the rotating plans
+    and timed with CUDA events on the launching stream (so it includes the launch gap, as the kernel
+    does inside the step; events recorded around every single launch would add microseconds)."""
     pat, torch = rig.pat, rig.torch
     for p in rig.plans:
-        pat.pat_set_profiling(p.handle, 1)
-    with torch.cuda.stream(rig.stream):
-        for i in range(nsteps):
-            rig.step(i)
-    torch.cuda.synchronize()
-    n = a = b = 0.0
+        pat.pat_set_profiling(p.handle, mode)
+    rig.capture_round()
+    ms = time_steps(rig, nsteps, warmup)
     for p in rig.plans:
-        c, pa, ga = pat.pat_get_profile(p.handle, True)
-        n, a, b = n + c, a + pa, b + ga
         pat.pat_set_profiling(p.handle, 0)
-    return (a / n, b / n) if n else (float("nan"), float("nan"))
+    rig.capture_round()
+    return ms / nsteps
 
 
 def measure(geom, tau, traces, B, steps, warmup, variant, dist, peak_gbs, sm_mhz, do_e2e):
@@ -269,7 +268,9 @@ def measure(geom, tau, traces, B, steps, warmup, variant, dist, peak_gbs, sm_mhz
     l0 = rig.launches()
     ms = time_steps(rig, steps, warmup, dist)
     per_step_launches = 2                                # pre-pass + gather per pat_backproject
-    pre_ms, gat_ms = profile_gather(rig, min(max(steps, rig.R), 512))
+    nk = max(rig.R, min(steps, 1000))
+    gat_ms = kernel_only_ms(rig, 2, nk, min(warmup, 20))
+    pre_ms = kernel_only_ms(rig, 3, nk, min(warmup, 20))
     out = {
         "B": B, "plans_rotated": rig.R, "ms_per_step": ms / steps, "ms_per_frame": ms / steps / B,
         "gupd_s": upd * steps / (ms * 1e-3) / 1e9,

@@ -133,11 +133,13 @@ int64_t pat_kernel_launches(const pat_plan *plan);
  * Results do not depend on the tuning beyond fp32 summation order. */
 pat_status pat_set_gather_tuning(pat_plan *plan, int32_t wr, int32_t rows, int32_t stages);
 
-/* Measurement helper (bench.py's roofline leg): while enabled, pat_backproject brackets the
- * pre-pass and the gather with CUDA events on `stream` (this disables their programmatic
- * overlap).  pat_get_profile waits for the recorded events and returns the number of profiled
- * calls and the summed device milliseconds of each kernel since the last reset; any out
- * pointer may be NULL.  At most 65536 calls are recorded between resets. */
+/* Measurement helper (bench.py's roofline leg).  mode 0 = off; 1 = pat_backproject brackets the
+ * pre-pass and the gather with CUDA events on `stream` (this disables their programmatic overlap and
+ * adds event overhead); 2 = pat_backproject launches ONLY the gather (b is whatever the last full
+ * call left; the images are not zeroed -- timing only); 3 = only the pre-pass.  pat_get_profile
+ * (mode 1) waits for the recorded events and returns the number of profiled calls and the summed
+ * device milliseconds of each kernel since the last reset; any out pointer may be NULL.  At most
+ * 65536 calls are recorded between resets. */
 pat_status pat_set_profiling(pat_plan *plan, int32_t enable);
 pat_status pat_get_profile(pat_plan *plan, int32_t reset, int64_t *calls, double *prepass_ms,
                            double *gather_ms);

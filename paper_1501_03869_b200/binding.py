@@ -163,8 +163,9 @@ def pat_set_gather_tuning(plan, wr=0, rows=0, stages=0):
     return _check(plan, lib().pat_set_gather_tuning(plan, wr, rows, stages))
 
 
-def pat_set_profiling(plan, enable):
-    return _check(plan, lib().pat_set_profiling(plan, int(enable)))
+def pat_set_profiling(plan, mode):
+    """0 off, 1 events per kernel, 2 gather only, 3 pre-pass only (see include/pat.h)."""
+    return _check(plan, lib().pat_set_profiling(plan, int(mode)))
 
 
 def pat_get_profile(plan, reset=True):

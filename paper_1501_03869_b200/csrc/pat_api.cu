@@ -446,7 +446,7 @@ extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *i
         pat_status ss = get_schedule(p, bp, &sc);
         if (ss != PAT_OK) return ss;
     }
-    const bool prof = p->profiling && p->prof_events.size() < 3u * 65536u;
+    const bool prof = p->profiling == 1 && p->prof_events.size() < 3u * 65536u;
     PatLaunchCtx ctx{stream, p->num_sms, p->use_pdl && !prof};
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
     if (prof) {
@@ -459,11 +459,14 @@ extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *i
     }
     float *bw = (float *)(p->ws + p->lay.bd);
     const float t0fs = (float)((double)p->t0 * (double)p->fs);
-    int e = pat_launch_prepass(ctx, d_tr, bw, d_img, d.nsens, d.nt, p->nt4, nframes, bp, d.npix, p->wp, p->wd, t0fs);
-    if (e) return cuda_fail(p, e, "pre-pass launch");
-    ++p->launches;
+    int e = 0;
+    if (p->profiling != 2) {
+        e = pat_launch_prepass(ctx, d_tr, bw, d_img, d.nsens, d.nt, p->nt4, nframes, bp, d.npix, p->wp, p->wd, t0fs);
+        if (e) return cuda_fail(p, e, "pre-pass launch");
+        ++p->launches;
+    }
     if (prof) cudaEventRecord(ev[1], st);
-    if (sc->grid_x > 0) {
+    if (sc->grid_x > 0 && p->profiling != 3) {
         e = pat_launch_gather(ctx, sc->cfg, (const float *)(p->ws + p->lay.tau), bw, sc->d_sched, sc->d_cta_chunk,
                               sc->grid_x, (const int32_t *)(p->ws + p->lay.perm), d_img, d.nsens, d.npix, d.nt,
                               p->nt4, nframes);
@@ -492,7 +495,8 @@ extern "C" pat_status pat_destroy(pat_plan *p) {
 
 extern "C" pat_status pat_set_profiling(pat_plan *p, int32_t enable) {
     if (!p) return PAT_ERR_INVALID_ARG;
-    p->profiling = enable != 0;
+    if (enable < 0 || enable > 3) return fail(p, PAT_ERR_INVALID_ARG, "profiling mode must be 0..3");
+    p->profiling = enable;
     return PAT_OK;
 }
 

@@ -81,7 +81,7 @@ struct pat_plan {
     std::vector<float> sensors;
     std::vector<int64_t> roi;         // empty => all nodes
     int64_t launches = 0;
-    bool profiling = false;
+    int profiling = 0;        // pat_set_profiling mode
     std::vector<void *> prof_events;  // cudaEvent_t triples: before pre-pass, between, after gather
     std::string err;
 };
