@@ -356,8 +356,10 @@ def run_reference(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "gpu_launches": 0,
-        "config": {"workload": "configs[%d] %s" % (k, geom.name), "nsens": geom.nsens, "npix": geom.npix,
-                   "nt": geom.nt, "frames_per_step": nf},
+        "config": {"workload": "configs[%d] %s: %d sensors x %d px, Nt=%d, %d frame(s)/step"
+                               % (k, geom.name, geom.nsens, geom.npix, geom.nt, Bcfg),
+                   "nsens": geom.nsens, "npix": geom.npix, "nt": geom.nt, "frames_per_step": Bcfg,
+                   "weighting": "p - t*dp/dt (Eq. 7)", "sampled_frames_per_step": nf},
         "cpu_baseline": {"value": val, "unit": "GUpd/s", "cores": host_cores(), "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": "GUpd/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
@@ -393,7 +395,8 @@ def run_ours(args):
     do_sweep = (not args.no_sweep) and world == 1 and k in (1, 2) and not args.batch
     nframes = 64 if do_sweep else max(B, 16 if (world == 1 and not args.no_cpu_baseline) else B)
     # every rank owns its own frames: the path shards over frames with no exchange (weak scaling)
-    geom, tau, traces = prepare_inputs(k, args.reduced, nframes, frame0=rank * nframes)
+    from paper_1501_03869_b200.sharding import rank_frame_range
+    geom, tau, traces = prepare_inputs(k, args.reduced, nframes, frame0=rank_frame_range(rank, world, nframes)[0])
 
     sampler = ClockSampler(local)
     sampler.start()
