@@ -84,3 +84,28 @@ def test_config3_large_full():
     tr = W.make_traces(geom, tau)
     ref = oracle.backproject(tau, tr, geom.fs, geom.t0, 1)
     assert_parity(gpu_backproject(geom, tau, tr), ref, "config3")
+
+
+@pytest.mark.slow
+def test_config4_shape_full_cube_analytic_tau_sampled_outputs():
+    """configs[4]'s image cube at full size (128^3 = 2 097 152 voxels, 8192 tiles) with an analytic
+    tau = dist/c0 table (conventional BP) for 192 hemisphere sensors -- the FMM table
+    of the full config needs hours of host CPU.  Outputs are checked on a seeded sample of voxels
+    the oracle computes one by one, plus the first and last tile."""
+    geom = W.make_geometry(4)
+    S = 192
+    sens = geom.sensors[:: geom.nsens // S][:S].astype(np.float64)
+    xyz = geom.roi_coords()
+    tau = np.empty((S, geom.npix), dtype=np.float32)
+    for i in range(S):
+        tau[i] = (np.sqrt(((xyz - sens[i][None, :]) ** 2).sum(axis=1)) / 1540.0).astype(np.float32)
+    rng = np.random.default_rng(44)
+    tr = rng.standard_normal((2, S, geom.nt)).astype(np.float32)
+    g2 = W.make_geometry(4)
+    g2.sensors = sens.astype(np.float32)
+    got = gpu_backproject(g2, tau, tr)
+    pick = np.unique(np.concatenate([np.arange(256), np.arange(geom.npix - 256, geom.npix),
+                                     rng.integers(0, geom.npix, size=4000)]))
+    ref = oracle.backproject(np.ascontiguousarray(tau[:, pick]), tr, geom.fs, geom.t0, 1)
+    assert_parity(got[:, pick], ref, "config4-shaped cube, sampled voxels")
+    assert np.all(np.isfinite(got))
