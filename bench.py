@@ -161,6 +161,8 @@ class Rig:
         l2 = getattr(props, "L2_cache_size", 126 << 20) or (126 << 20)
         step_bytes = algorithmic_bytes(geom.nsens, geom.npix, geom.nt, B)
         self.R = int(max(2, min(12, math.ceil(3.0 * l2 / step_bytes))))
+        if os.environ.get("PAT_BENCH_WARM_L2") == "1":     # diagnostic: one plan only, the table stays in L2
+            self.R = 1
         self.l2_bytes = int(l2)
         self.plans, self.tr, self.img = [], [], []
         F = traces.shape[0]
