@@ -189,3 +189,25 @@ def test_invalid_tuning_is_rejected():
             pat.pat_set_gather_tuning(plan.handle, *bad)
         assert ei.value.status == pat.PAT_ERR_INVALID_ARG
     plan.close()
+
+
+def test_image_buffer_guard_bands_stay_intact():
+    """compute-sanitizer is closed on this pool: check by hand that nothing is written outside
+    images[nframes][npix] (guard bands before and after, odd sizes, padded last tile)."""
+    import torch
+    import paper_1501_03869_b200 as pat
+    g = _geom(1001, 7, 80)
+    rng = np.random.default_rng(9)
+    tau = (rng.uniform(-3.0, 83.0, size=(7, 1001)) / FS).astype(np.float32)
+    for B in (1, 3, 33):
+        tr = rng.standard_normal((B, 7, 80)).astype(np.float32)
+        plan = pat.Plan(g.n, g.h, g.origin, g.c_map, g.sensors, g.roi_index, g.nt, FS, 0.0, max_batch=B)
+        plan.set_travel_times(tau)
+        guard = 4096
+        big = torch.full((guard + B * 1001 + guard,), 12345.0, dtype=torch.float32, device="cuda")
+        img = big[guard:guard + B * 1001].view(B, 1001)
+        plan.backproject(torch.from_numpy(tr).cuda(), img, B)
+        torch.cuda.synchronize()
+        assert torch.all(big[:guard] == 12345.0) and torch.all(big[guard + B * 1001:] == 12345.0)
+        assert_parity(img.cpu().numpy(), oracle.backproject(tau, tr, FS, 0.0, 1), "guarded images B=%d" % B)
+        plan.close()
