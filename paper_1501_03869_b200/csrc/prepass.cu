@@ -112,29 +112,46 @@ prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *_
     }
 }
 
-// Bp = 1: no transposition needed -- one thread per 4 consecutive samples, straight from global
-// memory (the +-1 neighbours come from L1), 16-byte stores.
+// Bp <= 4: no shared-memory transposition -- one thread per 4 consecutive samples of all BP frames,
+// straight from global memory (the +-1 neighbours come from L1), BP 16-byte stores.
+template <int BP>
 __global__ void __launch_bounds__(256)
-prepass_b1_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
-                  int32_t nsens, int32_t nt, int32_t nt4, int64_t npix, float wp, float wd, float t0fs) {
+prepass_small_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
+                     int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int64_t npix, float wp, float wd,
+                     float t0fs) {
     asm volatile("griddepcontrol.launch_dependents;");
     const int64_t gid = (int64_t)blockIdx.x * 256 + threadIdx.x, nthr = (int64_t)gridDim.x * 256;
-    for (int64_t q = gid; q < npix; q += nthr) images[q] = 0.0f;
+    for (int64_t q = gid; q < npix * nframes; q += nthr) images[q] = 0.0f;
     const int32_t quads = nt4 >> 2;
     for (int64_t q = gid; q < (int64_t)nsens * quads; q += nthr) {
         const int32_t s = (int32_t)(q / quads), n0 = (int32_t)(q - (int64_t)s * quads) << 2;
-        const float *p = traces + (int64_t)s * nt;
-        float w[6];                                        // p[n0-1 .. n0+4]
+        float o[4][BP];
 #pragma unroll
-        for (int j = 0; j < 6; ++j) {
-            const int32_t n = n0 - 1 + j;
-            w[j] = (n >= 0 && n < nt) ? __ldg(p + n) : 0.0f;
+        for (int f = 0; f < BP; ++f) {
+            const float *p = traces + ((int64_t)f * nsens + s) * nt;
+            float w[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};    // p[n0-1 .. n0+4]
+            if (f < nframes) {
+                if ((nt & 3) == 0) {                       // rows are 16-byte aligned: one vector load + 2 halo
+                    const float4 v = __ldg(reinterpret_cast<const float4 *>(p + n0));
+                    w[1] = v.x; w[2] = v.y; w[3] = v.z; w[4] = v.w;
+                    if (n0 > 0) w[0] = __ldg(p + n0 - 1);
+                    if (n0 + 4 < nt) w[5] = __ldg(p + n0 + 4);
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 6; ++j) {
+                        const int32_t n = n0 - 1 + j;
+                        if (n >= 0 && n < nt) w[j] = __ldg(p + n);
+                    }
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                o[j][f] = (f < nframes && n0 + j < nt) ? weight_at(w + j, n0 + j, nt, wp, wd, t0fs) : 0.0f;
         }
-        float4 o;
-        float *ov = reinterpret_cast<float *>(&o);
+        float4 *dst = reinterpret_cast<float4 *>(b + ((int64_t)s * nt4 + n0) * BP);
+        const float *flat = &o[0][0];                      // [sample][frame] = the output order
 #pragma unroll
-        for (int j = 0; j < 4; ++j) ov[j] = (n0 + j < nt) ? weight_at(w + j, n0 + j, nt, wp, wd, t0fs) : 0.0f;
-        *reinterpret_cast<float4 *>(b + (int64_t)s * nt4 + n0) = o;
+        for (int v = 0; v < BP; ++v) dst[v] = make_float4(flat[4 * v], flat[4 * v + 1], flat[4 * v + 2], flat[4 * v + 3]);
     }
 }
 
@@ -153,12 +170,17 @@ int pat_launch_retile(const PatLaunchCtx &ctx, const float *src, float *u_t, con
 int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, float *images,
                        int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp,
                        int64_t npix, float wp, float wd, float t0fs) {
-    if (bp == 1) {
+    if (bp <= 4) {
         const int64_t work = (int64_t)nsens * (nt4 >> 2);
         int64_t blocks = (work + 255) / 256;
         if (blocks > (int64_t)ctx.num_sms * 16) blocks = (int64_t)ctx.num_sms * 16;
-        prepass_b1_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)ctx.stream>>>(traces, b, images, nsens, nt, nt4,
-                                                                                  npix, wp, wd, t0fs);
+        cudaStream_t st = (cudaStream_t)ctx.stream;
+        if (bp == 1)
+            prepass_small_kernel<1><<<(unsigned)blocks, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs);
+        else if (bp == 2)
+            prepass_small_kernel<2><<<(unsigned)blocks, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs);
+        else
+            prepass_small_kernel<4><<<(unsigned)blocks, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs);
         return (int)cudaGetLastError();
     }
     int log2_bp = 0;
