@@ -130,6 +130,8 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
     std::vector<int32_t> cost;                       // per chunk: fixed part + slots
     int32_t chunk_cost = 6;
     if (const char *cc = std::getenv("PAT_CHUNK_COST")) chunk_cost = std::max(0, std::atoi(cc));
+    int32_t slow_cost = 5;                           // a slot of a checked chunk, in units of half a fast slot
+    if (const char *cc = std::getenv("PAT_SLOW_COST")) slow_cost = std::max(1, std::atoi(cc));
     const size_t per_chunk = (size_t)R + 1;
     try {
         list.reserve((size_t)(V / R + ntiles + 16) * per_chunk);
@@ -152,7 +154,15 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
                 pos += sl.len;
             }
             for (int32_t q = (int32_t)cur.size(); q < R; ++q) list.push_back(Entry{0, 0, 0, 0});
-            cost.push_back(chunk_cost + (int32_t)cur.size() * (fast ? 2 : 3));
+            // cost model (measured with the per-CTA timeline, PAT_TRACE_FILE): bytes moved -- 256 samples
+            // of u per slot plus its window -- plus a fixed part per chunk; checked chunks cost more per slot
+            // Bp <= 2 (HBM-bound).  For larger Bp the time goes with rows x frames (shared-memory bound).
+            int32_t cc = chunk_cost * 64;
+            if (cfg.bp <= 2)
+                for (const Slot &sl : cur) cc += (256 + sl.len) * (fast ? 2 : slow_cost) / 2;
+            else
+                cc += 128 * (int32_t)cur.size() * (fast ? 2 : 3);
+            cost.push_back(cc);
             cur.clear();
             used = 0;
         };
@@ -203,6 +213,23 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
     } catch (...) { return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
     if (list.size() / per_chunk > (size_t)INT32_MAX) return fail(p, PAT_ERR_UNSUPPORTED, "work list too long");
     sc.nchunks = (int64_t)(list.size() / per_chunk);
+    if (const char *fn = std::getenv("PAT_SCHED_DUMP")) {        // diagnostic: per-CTA share composition
+        if (FILE *f = std::fopen(fn, "w")) {
+            for (int64_t c = 0; c < G; ++c) {
+                int64_t nch = cta_chunk[c + 1] - cta_chunk[c], nsl = 0, nwin = 0, nfast = 0;
+                for (int64_t q = cta_chunk[c]; q < cta_chunk[c + 1]; ++q) {
+                    const Entry *h = &list[(size_t)q * per_chunk];
+                    nfast += h->z & 1;
+                    for (int v = 1; v <= R; ++v) {
+                        const uint32_t klen = ((uint32_t)h[v].z >> 16) & 0x7FFFu;
+                        if (klen) { ++nsl; nwin += (klen + 4) & ~3; }
+                    }
+                }
+                std::fprintf(f, "%lld %lld %lld %lld %lld\n", (long long)c, (long long)nch, (long long)nsl, (long long)nwin, (long long)nfast);
+            }
+            std::fclose(f);
+        }
+    }
     if (const char *dbg = std::getenv("PAT_DEBUG")) {
         if (dbg[0] == '1') {
             int64_t ns = 0, nc = 0, nreal = 0;
@@ -467,9 +494,15 @@ extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *i
     }
     if (prof) cudaEventRecord(ev[1], st);
     if (sc->grid_x > 0 && p->profiling != 3) {
+        if (std::getenv("PAT_TRACE_FILE") && !p->trace_dev && nframes <= 32) {   // diagnostic timeline
+            if (cudaMalloc((void **)&p->trace_dev, (size_t)sc->grid_x * 8 * sizeof(unsigned long long)) == cudaSuccess)
+                p->trace_ctas = sc->grid_x;
+            else
+                p->trace_dev = nullptr;
+        }
         e = pat_launch_gather(ctx, sc->cfg, (const float *)(p->ws + p->lay.tau), bw, sc->d_sched, sc->d_cta_chunk,
                               sc->grid_x, (const int32_t *)(p->ws + p->lay.perm), d_img, d.nsens, d.npix, d.nt,
-                              p->nt4, nframes);
+                              p->nt4, nframes, p->trace_ctas == sc->grid_x ? p->trace_dev : nullptr);
         if (e) return cuda_fail(p, e, "gather launch");
         ++p->launches;
     }
@@ -488,6 +521,14 @@ static void drop_events(pat_plan *p) {
 }
 
 extern "C" pat_status pat_destroy(pat_plan *p) {
+    if (p && p->trace_dev) {                   // PAT_TRACE_FILE: dump the per-CTA timeline of the last launch
+        std::vector<unsigned long long> h((size_t)p->trace_ctas * 8);
+        cudaDeviceSynchronize();
+        if (cudaMemcpy(h.data(), p->trace_dev, h.size() * 8, cudaMemcpyDeviceToHost) == cudaSuccess)
+            if (const char *fn = std::getenv("PAT_TRACE_FILE"))
+                if (FILE *f = std::fopen(fn, "wb")) { std::fwrite(h.data(), 8, h.size(), f); std::fclose(f); }
+        cudaFree(p->trace_dev);
+    }
     if (p) { drop_events(p); drop_schedules(p); }
     delete p;
     return PAT_OK;

@@ -15,9 +15,6 @@
 // contiguous run that a 1-D bulk async copy (TMA) can fetch.
 constexpr int kTilePix = 256;
 
-// The value written into tau_t for padding lanes: u = tau*fs is negative => contributes 0.
-#define PAT_TAU_PAD (-1.0f)
-
 struct PatDims {
     int32_t nsens = 0;
     int64_t npix = 0;
@@ -81,6 +78,8 @@ struct pat_plan {
     std::vector<float> sensors;
     std::vector<int64_t> roi;         // empty => all nodes
     int64_t launches = 0;
+    unsigned long long *trace_dev = nullptr;   // PAT_TRACE_FILE diagnostic: timeline of the last gather launch
+    int trace_ctas = 0;
     int profiling = 0;        // pat_set_profiling mode
     std::vector<void *> prof_events;  // cudaEvent_t triples: before pre-pass, between, after gather
     std::string err;
@@ -116,6 +115,7 @@ size_t pat_gather_smem_bytes(const PatGatherConfig &c);
 int pat_gather_occupancy(const PatGatherConfig &c, int *per_sm);
 int pat_launch_gather(const PatLaunchCtx &ctx, const PatGatherConfig &c, const float *u_t, const float *b,
                       const void *sched, const int32_t *cta_chunk, int grid_x, const int32_t *perm,
-                      float *images, int32_t nsens, int64_t npix, int32_t nt, int32_t nt4, int32_t nframes);
+                      float *images, int32_t nsens, int64_t npix, int32_t nt, int32_t nt4, int32_t nframes,
+                      unsigned long long *trace = nullptr);   // trace: per-CTA timeline, 8 x u64 per CTA, or NULL
 
 #endif  // PAT_INTERNAL_H_

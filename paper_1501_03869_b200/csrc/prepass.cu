@@ -12,16 +12,18 @@ namespace {
 
 // ---- table re-tiling: tau row-major [count][npix] -> u tile-major [tile][sensor][256] --------
 // u = fl32(fl32(tau - t0)*fs): H2's time -> sample mapping, two fp32 roundings (R8),
-// done once here instead of once per frame in the gather; padding lanes get u = -1 (invalid).
+// done once here instead of once per frame in the gather.
 __global__ void __launch_bounds__(256)
 retile_kernel(const float *__restrict__ src, float *__restrict__ u_t,
               const int32_t *__restrict__ perm, int32_t nsens, int64_t npix,
               int32_t sensor_begin, int32_t count, float fs, float t0) {
     const int64_t tile = blockIdx.x;
-    const int32_t slot = perm[tile * kTilePix + threadIdx.x];
+    const int32_t slot = perm[tile * kTilePix + threadIdx.x], first = perm[tile * kTilePix];
     for (int32_t r = blockIdx.y; r < count; r += gridDim.y) {
-        float v = PAT_TAU_PAD;
-        if (slot >= 0) v = __fmul_rn(__fsub_rn(__ldg(src + (int64_t)r * npix + slot), t0), fs);
+        // padding lanes of the last tile repeat the tile's first pixel: the row stays "all valid" (no
+        // test in the gather's fast path) and the lane's sum is simply never written (perm = -1)
+        const int32_t from = slot >= 0 ? slot : first;
+        const float v = __fmul_rn(__fsub_rn(__ldg(src + (int64_t)r * npix + from), t0), fs);
         u_t[(tile * nsens + sensor_begin + r) * kTilePix + threadIdx.x] = v;
     }
 }
