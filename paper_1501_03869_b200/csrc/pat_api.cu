@@ -108,13 +108,15 @@ struct Slot { int32_t row, sensor, s0, klen, len; bool whole, allvalid; };
 pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule **out) {
     const int64_t ntiles = p->dims.ntiles;
     const int32_t S = p->dims.nsens;
-    const int32_t step = cfg.wr - 4, R = cfg.R;
+    const int32_t step = cfg.step, R = cfg.R;
+    const bool blocked = pat_gather_blocked(cfg.bp);   // window units: 32-sample blocks (else samples)
+    const int32_t amask = blocked ? ~31 : ~3, ntb = (p->dims.nt + 31) / 32;
     const int32_t *meta = p->host_meta.data();
     if ((int64_t)S * p->nt4 > (int64_t)INT32_MAX) return fail(p, PAT_ERR_UNSUPPORTED, "nsens*nt exceeds 2^31");
     int64_t V = 0;
     for (int64_t r = 0; r < ntiles * S; ++r) {
         const int32_t kmin = meta[2 * r], kmax = meta[2 * r + 1] < 0 ? -1 : (meta[2 * r + 1] & 0x3FFFFFFF);
-        if (kmax >= kmin) V += (kmax + 1 - (kmin & ~3) + step - 1) / step;
+        if (kmax >= kmin) V += (kmax + 1 - (kmin & amask) + step - 1) / step;
     }
     PatSchedule sc;
     sc.cfg = cfg;
@@ -148,7 +150,7 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
             list.push_back(Entry{cur_tile, 0, flags, cur[0].row});
             int32_t pos = 0;
             for (const Slot &sl : cur) {
-                list.push_back(Entry{sl.row, sl.sensor * p->nt4 + sl.s0,
+                list.push_back(Entry{sl.row, blocked ? sl.sensor * ntb + (sl.s0 >> 5) : sl.sensor * p->nt4 + sl.s0,
                                      (int32_t)((uint32_t)pos | ((uint32_t)sl.klen << 16) | (contig ? 0x80000000u : 0u)),
                                      sl.s0});
                 pos += sl.len;
@@ -180,13 +182,17 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
                 const int32_t kmin = meta[2 * r], kmax = meta[2 * r + 1] < 0 ? -1 : (meta[2 * r + 1] & 0x3FFFFFFF);
                 if (kmax < kmin) continue;
                 const bool allvalid = (meta[2 * r + 1] >> 30) & 1;
-                const int32_t n0 = kmin & ~3, kend = kmax + 1;
+                const int32_t n0 = kmin & amask, kend = kmax + 1;
+                // window of a slot with k-range [s0, s0+klen): samples s0 .. s0+klen, in units
+                auto units = [&](int32_t s0, int32_t klen) {
+                    return blocked ? ((s0 + klen) >> 5) - (s0 >> 5) + 1 : (klen + 4) & ~3;
+                };
                 if (kend - n0 <= step) {
-                    add_slot((int32_t)t, Slot{(int32_t)r, s, n0, kend - n0, (kend - n0 + 4) & ~3, true, allvalid});
+                    add_slot((int32_t)t, Slot{(int32_t)r, s, n0, kend - n0, units(n0, kend - n0), true, allvalid});
                 } else {
                     for (int32_t s0 = n0; s0 < kend; s0 += step) {
                         const int32_t klen = std::min(step, kend - s0);
-                        rest.push_back(Slot{(int32_t)r, s, s0, klen, (klen + 4) & ~3, false, false});
+                        rest.push_back(Slot{(int32_t)r, s, s0, klen, units(s0, klen), false, false});
                     }
                 }
             }
@@ -274,7 +280,7 @@ PatLayout pat_layout(const PatDims &d) {
     L.meta = take((size_t)d.ntiles * d.nsens * 2 * sizeof(int32_t));
     const int bp = pat_frames_per_group(d.max_batch);
     const size_t padded = (size_t)(d.max_batch + bp - 1) / bp * bp;
-    L.bd = take(padded * d.nsens * ((d.nt + 3) / 4 * 4) * sizeof(float));
+    L.bd = take(padded * d.nsens * ((d.nt + 31) / 32 * 32) * sizeof(float));
     L.perm = take((size_t)d.ntiles * kTilePix * sizeof(int32_t));
     L.traces = take((size_t)d.max_batch * d.nsens * d.nt * sizeof(float));
     L.images = take((size_t)d.max_batch * d.npix * sizeof(float));

@@ -26,7 +26,7 @@ struct PatDims {
 struct PatLayout {            // byte offsets into the caller's workspace
     size_t tau = 0;           // float  [ntiles][nsens][256]   u = fl32(fl32(tau - t0)*fs), tile-major
     size_t meta = 0;          // int2   [ntiles*nsens]         {kmin, kmax} of each row
-    size_t bd = 0;            // float  [ngroups][nsens][nt4][Bp]   weighted traces b
+    size_t bd = 0;            // float  weighted traces b: [g][nsens][nt4][Bp] (Bp <= 2) or blocked [g][nsens][ntb][Bp][32]
     size_t perm = 0;          // int32  [ntiles*256]  slot -> position in roi list, -1 = pad
     size_t traces = 0;        // float  [max_batch][nsens][nt]    staging for host traces
     size_t images = 0;        // float  [max_batch][npix]         staging for host images
@@ -41,7 +41,8 @@ PatLayout pat_layout(const PatDims &d);
 struct PatGatherConfig {
     int bp = 0;               // frames per group: 1, 2, 4, ..., 64
     int wr = 0;               // longest window of one slot, samples (longer rows are split)
-    int cap = 0;              // window samples one stage holds for all its slots together
+    int step = 0;             // longest k-range of one slot (longer rows are split into segments of this)
+    int cap = 0;              // window units one stage holds for all its slots (samples; 32-sample blocks for Bp >= 4)
     int R = 0;                // slots per stage
     int stages = 0;
     uint32_t hdr_bytes = 0, stage_bytes = 0;
@@ -103,12 +104,14 @@ int pat_launch_row_meta(const PatLaunchCtx &ctx, const float *u_t, void *meta, i
 // H1: weighting pre-pass (Eq. 7 integrand at the sample times):
 //   traces[f][s][n] (fp32) -> b[((g*nsens + s)*nt4 + n)*bp + fl],  f = g*bp + fl; rows n >= nt and
 //   frames f >= nframes are zero.  Also zeroes images[nframes*npix] (the gather accumulates into it).
+// bp >= 4 writes the blocked layout b[((g*nsens + s)*ntb + n/32)*bp + fl][n%32] (ntb = ceil(nt/32)).
 int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, float *images,
                        int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp,
                        int64_t npix, float wp, float wd, float t0fs);
 
 // H2-H4: the gather (gather.cu).
 int pat_frames_per_group(int32_t nframes);
+bool pat_gather_blocked(int bp);       // trace layout [sensor][n/32][frame][32] instead of [sensor][n][frame]
 int pat_gather_wrmax(int bp);          // default / largest slot window for this frame-count class
 PatGatherConfig pat_gather_config(int bp, int wr, int R, int stages);   // 0 = choose automatically
 size_t pat_gather_smem_bytes(const PatGatherConfig &c);

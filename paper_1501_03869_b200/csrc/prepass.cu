@@ -2,8 +2,9 @@
 //
 // H1 (Eq. 7): the integrand p_i(t) - t*dp_i/dt evaluated at the sample times,
 //   b[n] = wp*p[n] - wd*(n + t0*fs)*D[n],  D = central difference (one-sided at the ends),
-// written frame-fastest, b[group][sensor][sample][Bp], so that the window of samples a pixel tile
-// can touch is ONE contiguous run for all frames of a group (a single bulk async copy in gather.cu).
+// written so that the window of samples a pixel tile can touch is ONE contiguous run for all frames of a
+// group (a single bulk async copy in gather.cu): [group][sensor][sample][Bp] for Bp <= 2, blocked
+// [group][sensor][sample/32][Bp][32] for Bp >= 4.
 #include "pat_internal.h"
 
 #include <cuda_runtime.h>
@@ -41,6 +42,7 @@ __device__ __forceinline__ float weight_at(const float *t, int32_t n, int32_t nt
     return wp * __fmaf_rn(-tn, D, pn);                     // wp*(p - tn*D); wp = wd is 1 or 2 (exact)
 }
 
+// Bp = 32 (interleaved layout [sensor][sample][32]): transposition through shared memory.
 // Block = (sample chunk, sensor, frame group).  The chunk of every frame of the group is read
 // coalesced along time into shared memory (+1 halo each side), then written frame-fastest.
 __global__ void __launch_bounds__(256)
@@ -114,7 +116,50 @@ prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *_
     }
 }
 
-// Bp <= 4: no shared-memory transposition -- one thread per 4 consecutive samples of all BP frames,
+// Bp = 4, 8, 16: the BLOCKED layout b[g][sensor][n/32][frame][32] (gather.cu, PPL == 3).  One thread per
+// (frame, sensor, 4 consecutive samples): reads straight from the traces (coalesced along time, the +-1
+// neighbours come from L1) and writes one 16-byte piece of a 128-byte block -- no transposition at all.
+__global__ void __launch_bounds__(256)
+prepass_blocked_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
+                       int32_t nsens, int32_t nt, int32_t ntb, int32_t nframes, int32_t log2_bp, int32_t groups,
+                       int64_t npix, float wp, float wd, float t0fs) {
+    asm volatile("griddepcontrol.launch_dependents;");
+    const int64_t gid = (int64_t)blockIdx.x * 256 + threadIdx.x, nthr = (int64_t)gridDim.x * 256;
+    for (int64_t q = gid; q < npix * nframes; q += nthr) images[q] = 0.0f;
+    const int32_t bp = 1 << log2_bp, quads = ntb * 8;
+    const int64_t per_frame = (int64_t)nsens * quads, total = per_frame * ((int64_t)groups << log2_bp);
+    for (int64_t q = gid; q < total; q += nthr) {
+        const int32_t f = (int32_t)(q / per_frame);
+        const int64_t r = q - (int64_t)f * per_frame;
+        const int32_t s = (int32_t)(r / quads), n0 = (int32_t)(r - (int64_t)s * quads) << 2;
+        float4 o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        if (f < nframes && n0 < nt) {
+            const float *p = traces + ((int64_t)f * nsens + s) * nt;
+            float w[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};    // p[n0-1 .. n0+4]
+            if ((nt & 3) == 0) {                           // rows are 16-byte aligned: one vector load + 2 halo
+                const float4 v = __ldg(reinterpret_cast<const float4 *>(p + n0));
+                w[1] = v.x; w[2] = v.y; w[3] = v.z; w[4] = v.w;
+                if (n0 > 0) w[0] = __ldg(p + n0 - 1);
+                if (n0 + 4 < nt) w[5] = __ldg(p + n0 + 4);
+            } else {
+#pragma unroll
+                for (int j = 0; j < 6; ++j) {
+                    const int32_t n = n0 - 1 + j;
+                    if (n >= 0 && n < nt) w[j] = __ldg(p + n);
+                }
+            }
+            float *ov = reinterpret_cast<float *>(&o);
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (n0 + j < nt) ov[j] = weight_at(w + j, n0 + j, nt, wp, wd, t0fs);
+        }
+        const int32_t g = f >> log2_bp, fl = f & (bp - 1);
+        float *dst = b + (((((int64_t)g * nsens + s) * ntb + (n0 >> 5)) << log2_bp) + fl) * 32 + (n0 & 31);
+        *reinterpret_cast<float4 *>(dst) = o;
+    }
+}
+
+// Bp <= 2 (layout [sensor][sample][Bp]): one thread per 4 consecutive samples of all BP frames,
 // straight from global memory (the +-1 neighbours come from L1), BP 16-byte stores.
 template <int BP>
 __global__ void __launch_bounds__(256)
@@ -172,21 +217,29 @@ int pat_launch_retile(const PatLaunchCtx &ctx, const float *src, float *u_t, con
 int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, float *images,
                        int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp,
                        int64_t npix, float wp, float wd, float t0fs) {
-    if (bp <= 4) {
+    if (bp <= 2) {
         const int64_t work = (int64_t)nsens * (nt4 >> 2);
         int64_t blocks = (work + 255) / 256;
         if (blocks > (int64_t)ctx.num_sms * 16) blocks = (int64_t)ctx.num_sms * 16;
         cudaStream_t st = (cudaStream_t)ctx.stream;
         if (bp == 1)
             prepass_small_kernel<1><<<(unsigned)blocks, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs);
-        else if (bp == 2)
-            prepass_small_kernel<2><<<(unsigned)blocks, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs);
         else
-            prepass_small_kernel<4><<<(unsigned)blocks, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs);
+            prepass_small_kernel<2><<<(unsigned)blocks, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs);
         return (int)cudaGetLastError();
     }
     int log2_bp = 0;
     while ((1 << log2_bp) < bp) ++log2_bp;
+    if (pat_gather_blocked(bp)) {
+        const int32_t groups = (nframes + bp - 1) / bp, ntb = (nt + 31) / 32;
+        const int64_t work = (int64_t)groups * bp * nsens * ntb * 8;
+        int64_t blocks = (work + 255) / 256;
+        if (blocks > (int64_t)ctx.num_sms * 32) blocks = (int64_t)ctx.num_sms * 32;
+        prepass_blocked_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)ctx.stream>>>(traces, b, images, nsens, nt, ntb,
+                                                                                      nframes, log2_bp, groups, npix, wp,
+                                                                                      wd, t0fs);
+        return (int)cudaGetLastError();
+    }
     int32_t ns = 8192 / bp;                                // samples per block (a power of two)
     if (ns > 1024) ns = 1024;
     while (ns > 4 && ns > nt4) ns >>= 1;
