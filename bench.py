@@ -430,7 +430,7 @@ def run_ours(args):
         probe = {"workload": "configs[4] reduced: %d sensors x %d voxels, Nt=%d, 1 frame/step" % (g4.nsens, g4.npix, g4.nt),
                  "ms_per_frame": round(m4["ms_per_frame"], 6), "gupd_s": round(m4["gupd_s"], 1),
                  "step_hbm_frac": round(m4["step_hbm_frac"], 4), "gather_hbm_frac": round(m4["gather_gbs"] / peak_gbs, 4),
-                 "full_size_result": "profiles/r01_config4_full.md (34.4 GB table: 5.92 ms/frame, 0.887 of the HBM peak)"}
+                 "full_size_result": "profiles/r01_config4_full.md (34.4 GB table: 6.26 ms/frame, 0.84 of the HBM peak)"}
     sampler.stop_flag = True
     sampler.join(timeout=2.0)
     clocks_main = sampler.summary()
