@@ -274,12 +274,15 @@ def measure(geom, tau, traces, B, steps, warmup, variant, dist, peak_gbs, sm_mhz
     nk = max(rig.R, min(steps, 1000))
     gat_ms = kernel_only_ms(rig, 2, nk, min(warmup, 20))
     pre_ms = kernel_only_ms(rig, 3, nk, min(warmup, 20))
+    # context for the roofline fraction: ONE kernel that only streams the step's footprint (table + b in,
+    # images out), same rotation, same graph harness -- what a launch of this size can reach at all
+    probe_ms = kernel_only_ms(rig, 4, nk, min(warmup, 20))
     out = {
         "B": B, "plans_rotated": rig.R, "ms_per_step": ms / steps, "ms_per_frame": ms / steps / B,
         "gupd_s": upd * steps / (ms * 1e-3) / 1e9,
         "step_bytes": abytes,
         "step_hbm_frac": abytes * steps / (ms * 1e-3) / 1e9 / peak_gbs,
-        "prepass_ms": pre_ms, "gather_ms": gat_ms,
+        "prepass_ms": pre_ms, "gather_ms": gat_ms, "stream_probe_ms": probe_ms,
         "gather_gbs": abytes / (gat_ms * 1e-3) / 1e9,
         "launches_per_step": per_step_launches,
         "direct_call_launches_seen": rig.launches() - l0,
@@ -461,7 +464,12 @@ def run_ours(args):
                      "kernel": "gather", "kernel_ms": main["gather_ms"], "prepass_ms": main["prepass_ms"],
                      "algorithmic_bytes_per_launch": main["step_bytes"],
                      "frac_of_nominal_8TBs": gather_gbs / NOMINAL_HBM_GBS,
-                     "step_frac": main["step_hbm_frac"], "sm_side_frac": main["sm_side_frac"]},
+                     "step_frac": main["step_hbm_frac"], "sm_side_frac": main["sm_side_frac"],
+                     # a kernel that does nothing but stream the same bytes, timed the same way
+                     "stream_probe": {"ms": main["stream_probe_ms"],
+                                      "gbs": main["step_bytes"] / (main["stream_probe_ms"] * 1e-3) / 1e9,
+                                      "frac": main["step_bytes"] / (main["stream_probe_ms"] * 1e-3) / 1e9 / peak_gbs,
+                                      "gather_vs_probe": main["stream_probe_ms"] / main["gather_ms"]}},
         "paper_context": "PAPER.md:79: 123.79 ms for 512 sensors x 21323 px on a Tesla C2075, transfers included",
     }
     if "e2e_gupd_s" in main:

@@ -136,7 +136,9 @@ pat_status pat_set_gather_tuning(pat_plan *plan, int32_t wr, int32_t rows, int32
 /* Measurement helper (bench.py's roofline leg).  mode 0 = off; 1 = pat_backproject brackets the
  * pre-pass and the gather with CUDA events on `stream` (this disables their programmatic overlap and
  * adds event overhead); 2 = pat_backproject launches ONLY the gather (b is whatever the last full
- * call left; the images are not zeroed -- timing only); 3 = only the pre-pass.  pat_get_profile
+ * call left; the images are not zeroed -- timing only); 3 = only the pre-pass; 4 = neither: ONE kernel
+ * that merely streams the step's footprint (u table + b in, images out; the images are garbage) -- the
+ * "what does a plain read of these bytes cost here" line beside the roofline.  pat_get_profile
  * (mode 1) waits for the recorded events and returns the number of profiled calls and the summed
  * device milliseconds of each kernel since the last reset; any out pointer may be NULL.  At most
  * 65536 calls are recorded between resets. */

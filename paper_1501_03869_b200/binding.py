@@ -164,7 +164,7 @@ def pat_set_gather_tuning(plan, wr=0, rows=0, stages=0):
 
 
 def pat_set_profiling(plan, mode):
-    """0 off, 1 events per kernel, 2 gather only, 3 pre-pass only (see include/pat.h)."""
+    """0 off, 1 events per kernel, 2 gather only, 3 pre-pass only, 4 stream probe (see include/pat.h)."""
     return _check(plan, lib().pat_set_profiling(plan, int(mode)))
 
 

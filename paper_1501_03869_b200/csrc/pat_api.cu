@@ -493,6 +493,13 @@ extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *i
     float *bw = (float *)(p->ws + p->lay.bd);
     const float t0fs = (float)((double)p->t0 * (double)p->fs);
     int e = 0;
+    if (p->profiling == 4) {          // measurement: the step's footprint (table + b in, images out) as a plain stream
+        e = pat_launch_stream_probe(ctx, p->ws + p->lay.tau, (int64_t)d.ntiles * kTilePix * d.nsens * 4,
+                                    bw, (int64_t)nframes * d.nsens * p->nt4 * 4, d_img, (int64_t)nframes * d.npix);
+        if (e) return cuda_fail(p, e, "stream probe launch");
+        ++p->launches;
+        return PAT_OK;
+    }
     if (p->profiling != 2) {
         e = pat_launch_prepass(ctx, d_tr, bw, d_img, d.nsens, d.nt, p->nt4, nframes, bp, d.npix, p->wp, p->wd, t0fs);
         if (e) return cuda_fail(p, e, "pre-pass launch");
@@ -542,7 +549,7 @@ extern "C" pat_status pat_destroy(pat_plan *p) {
 
 extern "C" pat_status pat_set_profiling(pat_plan *p, int32_t enable) {
     if (!p) return PAT_ERR_INVALID_ARG;
-    if (enable < 0 || enable > 3) return fail(p, PAT_ERR_INVALID_ARG, "profiling mode must be 0..3");
+    if (enable < 0 || enable > 4) return fail(p, PAT_ERR_INVALID_ARG, "profiling mode must be 0..4");
     p->profiling = enable;
     return PAT_OK;
 }

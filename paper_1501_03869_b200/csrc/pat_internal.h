@@ -109,6 +109,10 @@ int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, f
                        int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp,
                        int64_t npix, float wp, float wd, float t0fs);
 
+// Measurement only (pat_set_profiling mode 4): stream a_bytes + c_bytes in, nout floats out.
+int pat_launch_stream_probe(const PatLaunchCtx &ctx, const void *a, int64_t a_bytes, const void *c, int64_t c_bytes,
+                            float *out, int64_t nout);
+
 // H2-H4: the gather (gather.cu).
 int pat_frames_per_group(int32_t nframes);
 bool pat_gather_blocked(int bp);       // trace layout [sensor][n/32][frame][32] instead of [sensor][n][frame]
