@@ -18,6 +18,7 @@ CPU FMM (input preparation, untimed).  Prints ONE JSON line (rank 0):
   e2e          the same metric through the C-ABI with pinned HOST traces/images (H2D + D2H timed).
   cpu_baseline the oracle (oracle/pat_oracle.c) timed on this box's host cores, rank 0, N = 1.
   large_workload_probe  the same path on configs[4] reduced (537 MB table): the gather's steady-state rate.
+  offline_eikonal  (not part of the step) the tau table of the geometry solved on the GPU vs the CPU fast marching.
   sweep        B = 1..64 on the same geometry (N = 1 only): ms/frame, GUpd/s, HBM fraction and the
                SM-side (shared-memory bandwidth) fraction, because for B >~ 4 the path is not
                HBM-bound (DESIGN.md "Rooflines").
@@ -148,6 +149,36 @@ def prepare_inputs(k, reduced, nframes, frame0=0):
                              geom.roi_index, geom.npix, 0, geom.nsens, 1, tau, 0)
     traces = W.make_traces(geom, tau, frames=range(frame0, frame0 + nframes))
     return geom, tau, traces
+
+
+def eikonal_probe(geom):
+    """SURVEY.md 8(f) NEXT-2, off the timed path: the travel-time table of this geometry solved on the GPU
+    (fast sweeping, csrc/eikonal.cu) beside the library's CPU fast marching on the host cores (a sample of
+    the sensors), wall clock, and how far the two tables are apart."""
+    import torch
+    import paper_1501_03869_b200 as pat
+    grid = pat.PatGrid.make(geom.n, geom.h, geom.origin)
+    cm = np.ascontiguousarray(geom.c_map, dtype=np.float32).ravel()
+    S = geom.nsens
+    out = torch.empty((S, geom.npix), dtype=torch.float32, device="cuda")
+    best, rounds = None, 0
+    for _ in range(3):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        rounds = pat.pat_eikonal_travel_times_device(grid, cm, geom.sensors, S, geom.roi_index, geom.npix, 0, S, out)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    m = min(S, 64)
+    tau = np.empty((m, geom.npix), dtype=np.float32)
+    t0 = time.perf_counter()
+    pat.pat_fmm_travel_times(grid, cm, geom.sensors, S, geom.roi_index, geom.npix, 0, m, 1, tau, 0)
+    cpu = time.perf_counter() - t0
+    d = np.abs(out[:m].cpu().numpy().view(np.int32).astype(np.int64) - tau.view(np.int32).astype(np.int64))
+    return {"workload": "%d sensors on the %s grid (first-order upwind, fp64)" % (S, "x".join(str(v) for v in geom.n)),
+            "gpu_s": round(best, 4), "gpu_ms_per_sensor": round(best * 1e3 / S, 4), "rounds": int(rounds),
+            "cpu_fmm_ms_per_sensor": round(cpu * 1e3 / m, 4), "cpu_threads": os.cpu_count(), "cpu_sample_sensors": m,
+            "speedup_vs_cpu_fmm": round((cpu / m) / (best / S), 2), "max_ulp_vs_cpu_fmm": int(d.max())}
 
 
 class Rig:
@@ -434,6 +465,9 @@ def run_ours(args):
                  "ms_per_frame": round(m4["ms_per_frame"], 6), "gupd_s": round(m4["gupd_s"], 1),
                  "step_hbm_frac": round(m4["step_hbm_frac"], 4), "gather_hbm_frac": round(m4["gather_gbs"] / peak_gbs, 4),
                  "full_size_result": "profiles/r01_config4_full.md (34.4 GB table: 6.26 ms/frame, 0.84 of the HBM peak)"}
+    eik = None
+    if do_sweep:
+        eik = eikonal_probe(geom)
     sampler.stop_flag = True
     sampler.join(timeout=2.0)
     clocks_main = sampler.summary()
@@ -480,6 +514,8 @@ def run_ours(args):
         line["sweep"] = sweep
     if probe:
         line["large_workload_probe"] = probe
+    if eik:
+        line["offline_eikonal"] = eik
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(geom, tau, traces)
     tpath = os.path.join(ROOT, "profiles", "traffic.json")

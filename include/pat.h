@@ -163,6 +163,29 @@ pat_status pat_fmm_travel_times(const pat_grid *grid, const float *c_map,
  * have been given to pat_plan_create) in chunks and feed every row to pat_set_travel_times. */
 pat_status pat_compute_travel_times(pat_plan *plan, int32_t order, int32_t nthreads, void *stream);
 
+/* pat_eikonal_travel_times_device -- SURVEY.md 8(f) NEXT-2: the same first-order upwind system
+ * solved on the GPU by sensor-batched fast sweeping (csrc/eikonal.cu): Gauss-Seidel
+ * passes in the 2^ndim axis orderings, run level by level, one CTA per sensor, fp64, until a whole
+ * round changes nothing.  The fixed point is what fast marching computes; rows agree with
+ * pat_fmm_travel_times(order = 1) to fp32 rounding.
+ *   c_map, sensor_xyz, roi_index   HOST, as for pat_fmm_travel_times.
+ *   tau_out      DEVICE fp32 [count][npix], written on `stream`; the call synchronises `stream`.
+ *   max_rounds   cap on rounds of 2^ndim passes per sensor (<= 0: 64).
+ *   rounds_out   HOST, may be NULL: the largest number of rounds any sensor needed.
+ * Temporary device memory (one fp64 field per concurrent sensor) is allocated and freed inside.
+ * A sensor outside the grid / bad c_map -> PAT_ERR_INVALID_ARG; a sensor that did not converge within
+ * max_rounds -> PAT_ERR_BAD_STATE (tau_out then holds upper bounds). */
+pat_status pat_eikonal_travel_times_device(const pat_grid *grid, const float *c_map,
+                                           const float *sensor_xyz, int32_t nsens,
+                                           const int64_t *roi_index, int64_t npix,
+                                           int32_t sensor_begin, int32_t count, float *tau_out,
+                                           int32_t max_rounds, int32_t *rounds_out, void *stream);
+
+/* Convenience: pat_eikonal_travel_times_device on the plan's own grid / c_map / sensors, in chunks
+ * through the plan's staging buffer, every row handed to pat_set_travel_times on the device. */
+pat_status pat_compute_travel_times_gpu(pat_plan *plan, int32_t max_rounds, int32_t *rounds_out,
+                                        void *stream);
+
 #ifdef __cplusplus
 }
 #endif

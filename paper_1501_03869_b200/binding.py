@@ -84,6 +84,11 @@ def lib():
     L.pat_fmm_travel_times.argtypes = [gp, vp, vp, i32, vp, i64, i32, i32, i32, vp, i32]
     L.pat_compute_travel_times.restype = ctypes.c_int
     L.pat_compute_travel_times.argtypes = [vp, i32, i32, vp]
+    L.pat_eikonal_travel_times_device.restype = ctypes.c_int
+    L.pat_eikonal_travel_times_device.argtypes = [gp, vp, vp, i32, vp, i64, i32, i32, vp, i32,
+                                                  ctypes.POINTER(i32), vp]
+    L.pat_compute_travel_times_gpu.restype = ctypes.c_int
+    L.pat_compute_travel_times_gpu.argtypes = [vp, i32, ctypes.POINTER(i32), vp]
     _lib = L
     return L
 
@@ -188,6 +193,26 @@ def pat_compute_travel_times(plan, order=1, nthreads=0, stream=None):
     return _check(plan, lib().pat_compute_travel_times(plan, order, nthreads, _stream(stream)))
 
 
+def pat_eikonal_travel_times_device(grid, c_map, sensor_xyz, nsens, roi_index, npix, sensor_begin, count,
+                                    tau_out, max_rounds=0, stream=None):
+    """GPU fast-sweeping solve (include/pat.h); tau_out is a DEVICE fp32 [count][npix] tensor.
+    Returns the largest number of rounds any sensor needed."""
+    r = ctypes.c_int32()
+    st = lib().pat_eikonal_travel_times_device(ctypes.byref(grid), _addr(c_map), _addr(sensor_xyz), nsens,
+                                               _addr(roi_index) if roi_index is not None else None, npix,
+                                               sensor_begin, count, _addr(tau_out), int(max_rounds),
+                                               ctypes.byref(r), _stream(stream))
+    if st != PAT_OK:
+        raise PatError(st, "pat_eikonal_travel_times_device failed")
+    return r.value
+
+
+def pat_compute_travel_times_gpu(plan, max_rounds=0, stream=None):
+    r = ctypes.c_int32()
+    _check(plan, lib().pat_compute_travel_times_gpu(plan, int(max_rounds), ctypes.byref(r), _stream(stream)))
+    return r.value
+
+
 class Plan:
     """Owns a plan handle and its torch workspace tensor (device memory stays torch's)."""
 
@@ -217,6 +242,10 @@ class Plan:
 
     def compute_travel_times(self, order=1, nthreads=0, stream=None):
         return pat_compute_travel_times(self.handle, order, nthreads, stream)
+
+    def compute_travel_times_gpu(self, max_rounds=0, stream=None):
+        """First-order solve on the GPU (fast sweeping); returns the rounds the slowest sensor took."""
+        return pat_compute_travel_times_gpu(self.handle, max_rounds, stream)
 
     def backproject(self, traces, images, nframes=None, stream=None):
         nframes = int(traces.shape[0]) if nframes is None else nframes

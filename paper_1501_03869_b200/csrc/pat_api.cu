@@ -610,3 +610,27 @@ extern "C" pat_status pat_compute_travel_times(pat_plan *p, int32_t order, int32
     }
     return PAT_OK;
 }
+
+extern "C" pat_status pat_compute_travel_times_gpu(pat_plan *p, int32_t max_rounds, int32_t *rounds_out,
+                                                   void *stream) {
+    if (!p) return PAT_ERR_INVALID_ARG;
+    if (p->c_map.empty() || p->sensors.empty())
+        return fail(p, PAT_ERR_BAD_STATE, "plan was created without c_map / sensor_xyz");
+    float *stage = (float *)(p->ws + p->lay.tau_stage);
+    const int32_t rows = (int32_t)std::max<int64_t>(1, p->lay.stage_rows);
+    int32_t worst = 0;
+    for (int32_t s = 0; s < p->dims.nsens; s += rows) {
+        const int32_t m = std::min(rows, p->dims.nsens - s);
+        int32_t r = 0;
+        pat_status st = pat_eikonal_travel_times_device(&p->grid, p->c_map.data(), p->sensors.data(), p->dims.nsens,
+                                                        p->roi.empty() ? nullptr : p->roi.data(), p->dims.npix, s, m,
+                                                        stage, max_rounds, &r, stream);
+        if (st != PAT_OK) return fail(p, st, "pat_eikonal_travel_times_device failed (sensor outside the grid, or no convergence)");
+        worst = std::max(worst, r);
+        st = pat_set_travel_times(p, stage, s, m, stream);
+        if (st != PAT_OK) return st;
+        if (cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) return fail(p, PAT_ERR_CUDA, "synchronise");
+    }
+    if (rounds_out) *rounds_out = worst;
+    return PAT_OK;
+}
