@@ -106,6 +106,11 @@ pat_status pat_set_travel_times(pat_plan *plan, const float *tau, int32_t sensor
  * call with a given frame-count class (1, 2, 3-4, 5-8, 9-16, 17+) after the table changed, which
  * builds that class's work list (a few hundred KB of library-owned device memory, freed by
  * pat_destroy) and must therefore not happen inside a stream capture.
+ * HOST buffers (the paper's timings include the transfers): the traces are copied on a
+ * copy stream owned by the plan into one of two staging buffers and `stream` waits for that copy, so
+ * the transfer of one call runs under the kernels of the previous call; everything is complete when
+ * `stream` is (the host traces must stay untouched until then).  Inside a stream capture, or with
+ * PAT_NO_PIPE=1, the copy is simply enqueued on `stream`.
  * nframes = 0 is a no-op; nframes > max_batch -> PAT_ERR_INVALID_ARG; tau rows missing ->
  * PAT_ERR_BAD_STATE. */
 pat_status pat_backproject(pat_plan *plan, const float *traces, float *images,

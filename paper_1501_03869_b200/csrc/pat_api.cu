@@ -283,6 +283,7 @@ PatLayout pat_layout(const PatDims &d) {
     L.bd = take(padded * d.nsens * ((d.nt + 31) / 32 * 32) * sizeof(float));
     L.perm = take((size_t)d.ntiles * kTilePix * sizeof(int32_t));
     L.traces = take((size_t)d.max_batch * d.nsens * d.nt * sizeof(float));
+    L.traces2 = take((size_t)d.max_batch * d.nsens * d.nt * sizeof(float));
     L.images = take((size_t)d.max_batch * d.npix * sizeof(float));
     int64_t rows = (int64_t)((32u << 20) / ((size_t)d.npix * sizeof(float)));
     rows = std::max<int64_t>(1, std::min<int64_t>(rows, d.nsens));
@@ -399,6 +400,18 @@ extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, cons
     p->num_sms = sms;
     e = cudaMemcpy(p->ws + p->lay.perm, perm.data(), perm.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { delete p; return cuda_fail(nullptr, e, "upload of the pixel permutation"); }
+    if (!(std::getenv("PAT_NO_PIPE") && std::getenv("PAT_NO_PIPE")[0] == '1')) {
+        cudaStream_t cs = nullptr;
+        bool ok = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking) == cudaSuccess;
+        for (int q = 0; q < 2 && ok; ++q) {
+            cudaEvent_t a = nullptr, b = nullptr;
+            ok = cudaEventCreateWithFlags(&a, cudaEventDisableTiming) == cudaSuccess &&
+                 cudaEventCreateWithFlags(&b, cudaEventDisableTiming) == cudaSuccess;
+            p->ev_h2d[q] = a; p->ev_read[q] = b;
+        }
+        if (ok) p->copy_stream = cs;                   // otherwise host calls stay serial on the caller's stream
+        else if (cs) cudaStreamDestroy(cs);
+    }
     *out = p;
     return PAT_OK;
 }
@@ -466,12 +479,29 @@ extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *i
     const PatDims &d = p->dims;
     const float *d_tr = traces;
     float *d_img = images;
+    const int slot = (int)(p->host_calls & 1u);
+    bool piped = false;
     if (!td) {
-        d_tr = (const float *)(p->ws + p->lay.traces);
+        d_tr = (const float *)(p->ws + (slot ? p->lay.traces2 : p->lay.traces));
         d_img = (float *)(p->ws + p->lay.images);
-        cudaError_t e = cudaMemcpyAsync((void *)d_tr, traces, (size_t)nframes * d.nsens * d.nt * sizeof(float),
-                                        cudaMemcpyHostToDevice, st);
+        const size_t tbytes = (size_t)nframes * d.nsens * d.nt * sizeof(float);
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        cudaStreamIsCapturing(st, &cap);
+        piped = p->copy_stream && cap == cudaStreamCaptureStatusNone;
+        cudaError_t e;
+        if (piped) {
+            // the copy runs on the plan's copy stream, i.e. under the kernels of the previous call; it may
+            // overwrite this staging buffer once the pre-pass of the call before last has read it
+            cudaStream_t cs = (cudaStream_t)p->copy_stream;
+            e = p->host_calls >= 2 ? cudaStreamWaitEvent(cs, (cudaEvent_t)p->ev_read[slot], 0) : cudaSuccess;
+            if (e == cudaSuccess) e = cudaMemcpyAsync((void *)d_tr, traces, tbytes, cudaMemcpyHostToDevice, cs);
+            if (e == cudaSuccess) e = cudaEventRecord((cudaEvent_t)p->ev_h2d[slot], cs);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(st, (cudaEvent_t)p->ev_h2d[slot], 0);
+        } else {
+            e = cudaMemcpyAsync((void *)d_tr, traces, tbytes, cudaMemcpyHostToDevice, st);
+        }
         if (e != cudaSuccess) return cuda_fail(p, e, "traces H2D copy");
+        ++p->host_calls;
     }
     const int bp = pat_frames_per_group(nframes);
     PatSchedule *sc = nullptr;
@@ -506,6 +536,7 @@ extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *i
         ++p->launches;
     }
     if (prof) cudaEventRecord(ev[1], st);
+    if (piped) cudaEventRecord((cudaEvent_t)p->ev_read[slot], st);        // the staged traces have been consumed
     if (sc->grid_x > 0 && p->profiling != 3) {
         if (std::getenv("PAT_TRACE_FILE") && !p->trace_dev && nframes <= 32) {   // diagnostic timeline
             if (cudaMalloc((void **)&p->trace_dev, (size_t)sc->grid_x * 8 * sizeof(unsigned long long)) == cudaSuccess)
@@ -542,7 +573,14 @@ extern "C" pat_status pat_destroy(pat_plan *p) {
                 if (FILE *f = std::fopen(fn, "wb")) { std::fwrite(h.data(), 8, h.size(), f); std::fclose(f); }
         cudaFree(p->trace_dev);
     }
-    if (p) { drop_events(p); drop_schedules(p); }
+    if (p) {
+        drop_events(p); drop_schedules(p);
+        if (p->copy_stream) { cudaStreamSynchronize((cudaStream_t)p->copy_stream); cudaStreamDestroy((cudaStream_t)p->copy_stream); }
+        for (int q = 0; q < 2; ++q) {
+            if (p->ev_h2d[q]) cudaEventDestroy((cudaEvent_t)p->ev_h2d[q]);
+            if (p->ev_read[q]) cudaEventDestroy((cudaEvent_t)p->ev_read[q]);
+        }
+    }
     delete p;
     return PAT_OK;
 }

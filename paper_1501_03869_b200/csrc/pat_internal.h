@@ -29,6 +29,7 @@ struct PatLayout {            // byte offsets into the caller's workspace
     size_t bd = 0;            // float  weighted traces b: [g][nsens][nt4][Bp] (Bp <= 2) or blocked [g][nsens][ntb][Bp][32]
     size_t perm = 0;          // int32  [ntiles*256]  slot -> position in roi list, -1 = pad
     size_t traces = 0;        // float  [max_batch][nsens][nt]    staging for host traces
+    size_t traces2 = 0;       // float  second staging buffer: the copy of call i+1 overlaps the kernels of call i
     size_t images = 0;        // float  [max_batch][npix]         staging for host images
     size_t tau_stage = 0;     // float  [stage_rows][npix]        staging for host tau rows
     int64_t stage_rows = 0;
@@ -81,6 +82,11 @@ struct pat_plan {
     int64_t launches = 0;
     unsigned long long *trace_dev = nullptr;   // PAT_TRACE_FILE diagnostic: timeline of the last gather launch
     int trace_ctas = 0;
+    // host-buffer calls: H2D on an own copy stream into alternating staging buffers, so that the transfer
+    // of one call runs under the kernels of the previous one
+    void *copy_stream = nullptr;
+    void *ev_h2d[2] = {nullptr, nullptr}, *ev_read[2] = {nullptr, nullptr};
+    uint64_t host_calls = 0;
     int profiling = 0;        // pat_set_profiling mode
     std::vector<void *> prof_events;  // cudaEvent_t triples: before pre-pass, between, after gather
     std::string err;

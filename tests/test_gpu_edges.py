@@ -211,3 +211,28 @@ def test_image_buffer_guard_bands_stay_intact():
         assert torch.all(big[:guard] == 12345.0) and torch.all(big[guard + B * 1001:] == 12345.0)
         assert_parity(img.cpu().numpy(), oracle.backproject(tau, tr, FS, 0.0, 1), "guarded images B=%d" % B)
         plan.close()
+
+
+def test_host_calls_back_to_back_overlap_copies_and_kernels():
+    """Host-buffer calls stage their traces through two alternating buffers on the plan's copy stream
+    (the transfer of call i+1 runs under the kernels of call i).  Six calls without a synchronise in
+    between, different traces each: every image must be the one of its own traces."""
+    import torch
+    import paper_1501_03869_b200 as pat
+    g = _geom(1500, 24, 256)
+    rng = np.random.default_rng(21)
+    tau = (rng.uniform(2.0, 250.0, size=(24, 1500)) / FS).astype(np.float32)
+    plan = pat.Plan(g.n, g.h, g.origin, g.c_map, g.sensors, g.roi_index, g.nt, FS, 0.0, max_batch=2)
+    try:
+        plan.set_travel_times(tau)
+        trs = [torch.from_numpy(rng.standard_normal((2, 24, 256)).astype(np.float32)).pin_memory() for _ in range(6)]
+        imgs = [torch.empty((2, 1500), dtype=torch.float32).pin_memory() for _ in range(6)]
+        st = torch.cuda.Stream()
+        for tr, im in zip(trs, imgs):
+            plan.backproject(tr, im, 2, st)
+        st.synchronize()
+        for q, (tr, im) in enumerate(zip(trs, imgs)):
+            ref = oracle.backproject(tau, tr.numpy(), FS, 0.0, 1)
+            assert_parity(im.numpy(), ref, "back-to-back host call %d" % q)
+    finally:
+        plan.close()
