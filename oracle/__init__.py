@@ -28,6 +28,8 @@ def lib():
         L.oracle_fmm.argtypes = [i32, vp, f64, vp, vp, vp, i32, vp, vp]
         L.oracle_fmm_rows.restype = ctypes.c_int
         L.oracle_fmm_rows.argtypes = [i32, vp, f64, vp, vp, vp, i32, vp, i64, i32, vp]
+        L.oracle_tau_conventional.restype = ctypes.c_int
+        L.oracle_tau_conventional.argtypes = [i32, vp, f32, vp, vp, i32, vp, i64, f32, vp]
         L.oracle_weight.restype = None
         L.oracle_weight.argtypes = [vp, i32, f64, f64, f64, vp]
         L.oracle_backproject.restype = ctypes.c_int
@@ -72,6 +74,22 @@ def fmm_rows(n, h, origin, c_map, sensors, roi_index, order=1):
                                _p(roi), roi.size, int(order), _p(tau))
     if rc:
         raise ValueError("oracle_fmm_rows failed with code %d" % rc)
+    return tau
+
+
+def tau_conventional(n, h, origin, sensors, roi_index, c0):
+    """tau[i][j] fp32 = |r_j - s_i| / c0 in the fp32 operation order the oracle fixes."""
+    ndim = len(n)
+    n3 = np.array(list(n) + [1] * (3 - ndim), dtype=np.int32)
+    org = np.array(list(origin) + [0.0] * (3 - len(origin)), dtype=np.float32)
+    sens = np.ascontiguousarray(sensors, dtype=np.float32).reshape(-1, 3)
+    roi = None if roi_index is None else np.ascontiguousarray(roi_index, dtype=np.int64)
+    npix = int(np.prod(n3)) if roi is None else roi.size
+    tau = np.empty((sens.shape[0], npix), dtype=np.float32)
+    rc = lib().oracle_tau_conventional(ndim, _p(n3), float(np.float32(h)), _p(org), _p(sens), sens.shape[0],
+                                       _p(roi) if roi is not None else None, npix, float(np.float32(c0)), _p(tau))
+    if rc:
+        raise ValueError("oracle_tau_conventional failed with code %d" % rc)
     return tau
 
 

@@ -8,6 +8,7 @@
  *   oracle_fmm          eikonal arrival times, PAPER.md:49-58 (Sec. II.B, Eq. 5)
  *   oracle_weight       the integrand of Eq. 7 at the sample times
  *   oracle_backproject  Eq. 7 as a plain triple loop, PAPER.md:64-69 (Sec. II.C)
+ *   oracle_tau_conventional  the conventional BP's analytic delays
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
  * reference legs may call this file.  It shares no code, header, table or
@@ -284,6 +285,47 @@ int oracle_fmm_rows(int32_t ndim, const int32_t *n, double h, const double *orig
 /* ------------------------------------------------------------------------- */
 /* Eq. 7:  P(r_j) = sum_i [ p_i(t_ij) - t_ij * dp_i/dt (t_ij) ] */
 /* ------------------------------------------------------------------------- */
+
+/* oracle_tau_conventional: the conventional back projection's delays
+ * ("In the conventional BP algorithm, t_ij is calculated
+ * analytically by assuming a constant speed"): tau_ij = |r_j - s_i| / c0, with
+ * r_j the position of ROI node j and s_i the sensor position.  The delay goes
+ * through floor() in Eq. 7's time -> sample map, so its arithmetic type is part
+ * of the definition (R26): fp32, one IEEE operation per step, in the
+ * order
+ *     x_d  = fl(origin_d + fl((float)i_d * h))          node coordinate, axis d
+ *     e_d  = fl(x_d - s_d)
+ *     d2   = fl(fl(fl(e_0*e_0) + fl(e_1*e_1)) + fl(e_2*e_2))   (no e_2 term in 2-D)
+ *     tau  = fl(fl(sqrt(d2)) * fl(1/c0))
+ * (-ffp-contract=off: no fused multiply-add).  sensors: fp32 [nsens][3];
+ * roi: linear node indices (x fastest) or NULL for all nodes; tau: fp32
+ * [nsens][npix].  Returns 0, or 1 for a bad argument. */
+int oracle_tau_conventional(int32_t ndim, const int32_t *n, float h, const float *origin,
+                            const float *sensors, int32_t nsens, const int64_t *roi,
+                            int64_t npix, float c0, float *tau)
+{
+    if ((ndim != 2 && ndim != 3) || !n || !origin || !sensors || !tau || !(c0 > 0.0f)) return 1;
+    const int64_t n0 = n[0], n1 = n[1];
+    const float inv_c0 = 1.0f / c0;
+    for (int32_t i = 0; i < nsens; ++i) {
+        const float *s = sensors + 3 * (int64_t)i;
+        for (int64_t j = 0; j < npix; ++j) {
+            const int64_t q = roi ? roi[j] : j;
+            const int64_t id[3] = { q % n0, (q / n0) % n1, q / (n0 * n1) };
+            float d2 = 0.0f;
+            for (int d = 0; d < ndim; ++d) {
+                const float step = (float)id[d] * h;
+                const float x = origin[d] + step;
+                const float e = x - s[d];
+                const float sq = e * e;
+                d2 = d == 0 ? sq : d2 + sq;
+            }
+            const float dist = sqrtf(d2);
+            tau[(int64_t)i * npix + j] = dist * inv_c0;
+        }
+    }
+    return 0;
+}
 
 /* oracle_weight: b[n] = wp*p[n] - wd*t_n*(dp/dt)[n] at the sample times
  * t_n = t0 + n/fs.  With the finite difference D[n] (central, one-sided at the

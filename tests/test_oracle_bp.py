@@ -226,3 +226,53 @@ def test_pitch_and_empty_inputs():
     wide[:, :20] = tau
     np.testing.assert_array_equal(oracle.backproject(wide[:, :20], tr, FS), oracle.backproject(tau, tr, FS))
     assert oracle.backproject(tau[:, :0], tr, FS).shape == (1, 0)
+
+
+# ---- P15: the conventional BP's analytic delays -------------------------------------
+def test_tau_conventional_matches_the_closed_form_and_its_invariants():
+    """oracle.tau_conventional against |r - s| / c0 written out in fp64 from the SAME fp32-rounded node
+    coordinates (what is pinned is the formula and the index -> coordinate map, x fastest); a transposed
+    axis, a missing square root, c0 instead of 1/c0 or a dropped axis all fail here."""
+    rng = np.random.default_rng(2)
+    for n, origin in [((13, 9), (-6.0e-4, 2.0e-4)), ((7, 5, 6), (1.0e-4, -3.0e-4, 0.0))]:
+        h, c0 = np.float32(1.0e-4), np.float32(1560.0)
+        N = int(np.prod(n))
+        roi = np.sort(rng.choice(N, size=N // 2, replace=False)).astype(np.int64)
+        sens = np.zeros((4, 3), dtype=np.float32)
+        for d in range(len(n)):
+            sens[:, d] = np.float32(origin[d]) + rng.uniform(-3, n[d] + 3, size=4).astype(np.float32) * h
+        tau = oracle.tau_conventional(n, h, origin, sens, roi, c0)
+        assert tau.shape == (4, roi.size) and tau.dtype == np.float32
+        idx = np.stack(np.unravel_index(roi, n[::-1]), axis=1)[:, ::-1]          # (i0, i1[, i2]), x fastest
+        x32 = (np.asarray(origin, np.float32)[None, :] + (idx.astype(np.float32) * h)).astype(np.float32)
+        for i in range(4):
+            e = x32.astype(np.float64) - sens[i, :len(n)].astype(np.float64)[None, :]
+            want = np.sqrt((e * e).sum(axis=1)) / float(c0)
+            np.testing.assert_allclose(tau[i].astype(np.float64), want, rtol=6 * 2.0 ** -24, atol=0.0)
+    # a sensor sitting on a node: that node's delay is exactly 0, its axis neighbours' exactly h/c0 (to rounding)
+    n, h, c0 = (9, 9), np.float32(0.5), np.float32(2.0)
+    sens = np.array([[2.0, 1.5, 0.0]], dtype=np.float32)                         # node (4, 3) with origin 0
+    tau = oracle.tau_conventional(n, h, (0.0, 0.0), sens, None, c0).reshape(9, 9)
+    assert tau[3, 4] == 0.0
+    assert tau[3, 5] == tau[3, 3] == tau[4, 4] == tau[2, 4] == np.float32(0.25)
+    assert tau[0, 0] == np.float32(np.sqrt(np.float32(2.0 * 2.0 + 1.5 * 1.5))) * np.float32(0.5)
+
+
+def test_conventional_bp_point_source_focuses_at_the_source():
+    """End to end (Eq. 7 with analytic delays): traces that carry one pulse at |r* - s_i|/c0
+    back-project to an image whose maximum sits on the node r*."""
+    n, h, c0, fs, nt = (31, 31), np.float32(1.0e-4), np.float32(1500.0), 40.0e6, 256
+    ang = np.linspace(0, 2 * np.pi, 24, endpoint=False)
+    sens = np.zeros((24, 3), dtype=np.float32)
+    sens[:, 0] = 1.5e-3 + 4.0e-3 * np.cos(ang)
+    sens[:, 1] = 1.5e-3 + 4.0e-3 * np.sin(ang)
+    src = (19, 11)
+    rs = np.array([src[0] * float(h), src[1] * float(h)])
+    tr = np.zeros((1, 24, nt), dtype=np.float32)
+    for i in range(24):
+        k = int(round(np.hypot(*(rs - sens[i, :2].astype(np.float64))) / float(c0) * fs))
+        tr[0, i, k] = 1.0
+    tau = oracle.tau_conventional(n, h, (0.0, 0.0), sens, None, c0)
+    img = oracle.backproject(tau, tr, fs, 0.0, 0)                               # plain delay and sum
+    j = int(np.argmax(img[0]))
+    assert (j % 31, j // 31) == src
