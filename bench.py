@@ -18,6 +18,7 @@ CPU FMM (input preparation, untimed).  Prints ONE JSON line (rank 0):
   e2e          the same metric through the C-ABI with pinned HOST traces/images (H2D + D2H timed).
   cpu_baseline the oracle (oracle/pat_oracle.c) timed on this box's host cores, rank 0, N = 1.
   large_workload_probe  the same path on configs[4] reduced (537 MB table): the gather's steady-state rate.
+  conventional_bp  PAPER.md:69's comparison method with the delays computed in the kernel (no table stream).
   offline_eikonal  (not part of the step) the tau table of the geometry solved on the GPU vs the CPU fast marching.
   sweep        B = 1..64 on the same geometry (N = 1 only): ms/frame, GUpd/s, HBM fraction and the
                SM-side (shared-memory bandwidth) fraction, because for B >~ 4 the path is not
@@ -179,6 +180,44 @@ def eikonal_probe(geom):
             "gpu_s": round(best, 4), "gpu_ms_per_sensor": round(best * 1e3 / S, 4), "rounds": int(rounds),
             "cpu_fmm_ms_per_sensor": round(cpu * 1e3 / m, 4), "cpu_threads": os.cpu_count(), "cpu_sample_sensors": m,
             "speedup_vs_cpu_fmm": round((cpu / m) / (best / S), 2), "max_ulp_vs_cpu_fmm": int(d.max())}
+
+
+def conventional_probe(geom, traces, batches=(1, 32)):
+    """the conventional BP (tau = |r - s|/c0 computed in the gather) on the
+    same geometry.  No table stream, so the kernel is bound by arithmetic, not HBM; timed from a CUDA graph of
+    16 calls (traces resident, 4 MB/frame: they would fit L2 in any harness)."""
+    import torch
+    import paper_1501_03869_b200 as pat
+    out = []
+    for B in batches:
+        tr = torch.from_numpy(np.ascontiguousarray(np.resize(traces, (B,) + traces.shape[1:]))).cuda()
+        img = torch.empty((B, geom.npix), dtype=torch.float32, device="cuda")
+        plan = pat.Plan(geom.n, geom.h, geom.origin, geom.c_map, geom.sensors, geom.roi_index, geom.nt, geom.fs,
+                        geom.t0, max_batch=B)
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            plan.backproject_conventional(tr, img, 1560.0, B, st)            # set-up outside the capture
+            st.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=st):
+                for _ in range(16):
+                    plan.backproject_conventional(tr, img, 1560.0, B, st)
+            for _ in range(3):
+                g.replay()
+            st.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            reps = 20 if B == 1 else 4
+            e0.record(st)
+            for _ in range(reps):
+                g.replay()
+            e1.record(st)
+            st.synchronize()
+        ms = e0.elapsed_time(e1) / (16 * reps)
+        upd = float(B) * geom.nsens * geom.npix
+        out.append({"B": B, "c0": 1560.0, "ms_per_frame": round(ms / B, 6), "gupd_s": round(upd / (ms * 1e-3) / 1e9, 1)})
+        del g
+        plan.close()
+    return out
 
 
 class Rig:
@@ -465,9 +504,10 @@ def run_ours(args):
                  "ms_per_frame": round(m4["ms_per_frame"], 6), "gupd_s": round(m4["gupd_s"], 1),
                  "step_hbm_frac": round(m4["step_hbm_frac"], 4), "gather_hbm_frac": round(m4["gather_gbs"] / peak_gbs, 4),
                  "full_size_result": "profiles/r01_config4_full.md (34.4 GB table: 6.26 ms/frame, 0.84 of the HBM peak)"}
-    eik = None
+    eik, conv = None, None
     if do_sweep:
         eik = eikonal_probe(geom)
+        conv = conventional_probe(geom, traces)
     sampler.stop_flag = True
     sampler.join(timeout=2.0)
     clocks_main = sampler.summary()
@@ -516,6 +556,8 @@ def run_ours(args):
         line["large_workload_probe"] = probe
     if eik:
         line["offline_eikonal"] = eik
+    if conv:
+        line["conventional_bp"] = conv
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(geom, tau, traces)
     tpath = os.path.join(ROOT, "profiles", "traffic.json")

@@ -116,6 +116,18 @@ pat_status pat_set_travel_times(pat_plan *plan, const float *tau, int32_t sensor
 pat_status pat_backproject(pat_plan *plan, const float *traces, float *images,
                            int32_t nframes, void *stream);
 
+/* pat_backproject_conventional -- SURVEY.md 8(f) NEXT-3: the conventional back projection the paper
+ * compares with ("t_ij is calculated analytically by assuming a constant speed"; PAPER.md:79:
+ * c0 = 1560 m/s): Eq. 7 exactly as pat_backproject, but with tau_ij = |r_j - s_i| / c0 computed inside the
+ * gather instead of read from the table (no 4*S*P-byte stream: the kernel is arithmetic-bound).  r_j is the
+ * position of ROI node j on the plan's grid, s_i the plan's sensor position; fp32, one IEEE operation per
+ * step: x_d = origin_d + i_d*h, e_d = x_d - s_d, d2 = (e_0^2 + e_1^2) + e_2^2, tau = sqrt(d2) * (1/c0).
+ * The plan needs sensor_xyz but no travel-time table; tables and conventional calls may be mixed.
+ * The first call for a given c0 (and frame-count class) builds work lists and synchronises `stream`.
+ * Errors as pat_backproject; c0 not finite or <= 0 -> PAT_ERR_INVALID_ARG; no sensor_xyz -> PAT_ERR_BAD_STATE. */
+pat_status pat_backproject_conventional(pat_plan *plan, const float *traces, float *images,
+                                        int32_t nframes, float c0, void *stream);
+
 /* Frees the host-side plan; never frees caller memory.  NULL is allowed. */
 pat_status pat_destroy(pat_plan *plan);
 

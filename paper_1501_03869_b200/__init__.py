@@ -10,6 +10,7 @@ from .binding import (PAT_OK, PAT_ERR_INVALID_ARG, PAT_ERR_BAD_STATE, PAT_ERR_CU
                       pat_set_travel_times, pat_backproject, pat_destroy, pat_last_error,
                       pat_kernel_launches, pat_set_gather_tuning, pat_fmm_travel_times,
                       pat_compute_travel_times, pat_set_profiling, pat_get_profile,
-                      pat_eikonal_travel_times_device, pat_compute_travel_times_gpu, Plan)
+                      pat_eikonal_travel_times_device, pat_compute_travel_times_gpu,
+                      pat_backproject_conventional, Plan)
 
 __all__ = [n for n in dir() if n.startswith(("pat_", "PAT_", "Pat", "Plan", "lib"))]

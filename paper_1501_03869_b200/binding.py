@@ -84,6 +84,8 @@ def lib():
     L.pat_fmm_travel_times.argtypes = [gp, vp, vp, i32, vp, i64, i32, i32, i32, vp, i32]
     L.pat_compute_travel_times.restype = ctypes.c_int
     L.pat_compute_travel_times.argtypes = [vp, i32, i32, vp]
+    L.pat_backproject_conventional.restype = ctypes.c_int
+    L.pat_backproject_conventional.argtypes = [vp, vp, vp, i32, ctypes.c_float, vp]
     L.pat_eikonal_travel_times_device.restype = ctypes.c_int
     L.pat_eikonal_travel_times_device.argtypes = [gp, vp, vp, i32, vp, i64, i32, i32, vp, i32,
                                                   ctypes.POINTER(i32), vp]
@@ -152,6 +154,12 @@ def pat_backproject(plan, traces, images, nframes, stream=None):
     return _check(plan, lib().pat_backproject(plan, _addr(traces), _addr(images), nframes, _stream(stream)))
 
 
+def pat_backproject_conventional(plan, traces, images, nframes, c0, stream=None):
+    """Eq. 7 with tau = |r - s| / c0 computed in the kernel."""
+    return _check(plan, lib().pat_backproject_conventional(plan, _addr(traces), _addr(images), nframes,
+                                                           float(c0), _stream(stream)))
+
+
 def pat_destroy(plan):
     return lib().pat_destroy(plan)
 
@@ -217,13 +225,13 @@ class Plan:
     """Owns a plan handle and its torch workspace tensor (device memory stays torch's)."""
 
     def __init__(self, n, h, origin, c_map, sensor_xyz, roi_index, nt, fs, t0=0.0,
-                 weighting=PAT_W_PAPER, max_batch=1, device="cuda"):
+                 weighting=PAT_W_PAPER, max_batch=1, device="cuda", nsens=None):
         import torch
         self.grid = PatGrid.make(n, h, origin)
         self.c_map = None if c_map is None else np.ascontiguousarray(c_map, dtype=np.float32).ravel()
         self.sensor_xyz = None if sensor_xyz is None else np.ascontiguousarray(sensor_xyz, dtype=np.float32)
         self.roi_index = None if roi_index is None else np.ascontiguousarray(roi_index, dtype=np.int64)
-        self.nsens = int(self.sensor_xyz.shape[0]) if self.sensor_xyz is not None else None
+        self.nsens = int(self.sensor_xyz.shape[0]) if self.sensor_xyz is not None else int(nsens)
         self.npix = int(self.roi_index.size) if self.roi_index is not None else int(np.prod(n))
         self.nt, self.fs, self.t0, self.max_batch = int(nt), float(fs), float(t0), int(max_batch)
         nbytes = pat_plan_workspace_bytes(self.grid, self.nsens, self.npix, self.nt, self.max_batch)
@@ -250,6 +258,10 @@ class Plan:
     def backproject(self, traces, images, nframes=None, stream=None):
         nframes = int(traces.shape[0]) if nframes is None else nframes
         return pat_backproject(self.handle, traces, images, nframes, stream)
+
+    def backproject_conventional(self, traces, images, c0, nframes=None, stream=None):
+        nframes = int(traces.shape[0]) if nframes is None else nframes
+        return pat_backproject_conventional(self.handle, traces, images, nframes, c0, stream)
 
     def launches(self):
         return pat_kernel_launches(self.handle)

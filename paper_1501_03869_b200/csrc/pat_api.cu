@@ -111,7 +111,7 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
     const int32_t step = cfg.step, R = cfg.R;
     const bool blocked = pat_gather_blocked(cfg.bp);   // window units: 32-sample blocks (else samples)
     const int32_t amask = blocked ? ~31 : ~3, ntb = (p->dims.nt + 31) / 32;
-    const int32_t *meta = p->host_meta.data();
+    const int32_t *meta = cfg.onfly ? p->onfly_meta.data() : p->host_meta.data();
     if ((int64_t)S * p->nt4 > (int64_t)INT32_MAX) return fail(p, PAT_ERR_UNSUPPORTED, "nsens*nt exceeds 2^31");
     int64_t V = 0;
     for (int64_t r = 0; r < ntiles * S; ++r) {
@@ -146,6 +146,7 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
                 fast = fast && cur[q].whole && cur[q].allvalid;
                 contig = contig && cur[q].row == cur[0].row + (int32_t)q;
             }
+            if (cfg.onfly) contig = true;              // no u copies at all: the consumers compute u
             const int32_t flags = (fast ? 1 : 0) | (contig ? 2 : 0) | ((int32_t)cur.size() << 8);
             list.push_back(Entry{cur_tile, 0, flags, cur[0].row});
             int32_t pos = 0;
@@ -263,11 +264,72 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
     return PAT_OK;
 }
 
-pat_status get_schedule(pat_plan *p, int bp, PatSchedule **out) {
+pat_status get_schedule(pat_plan *p, int bp, bool onfly, PatSchedule **out) {
     for (PatSchedule &sc : p->schedules)
-        if (sc.cfg.bp == bp) { *out = &sc; return PAT_OK; }
-    PatGatherConfig cfg = pat_gather_config(bp, p->tune_wr, p->tune_R, p->tune_stages);
+        if (sc.cfg.bp == bp && sc.cfg.onfly == onfly) { *out = &sc; return PAT_OK; }
+    PatGatherConfig cfg = pat_gather_config(bp, p->tune_wr, p->tune_R, p->tune_stages, onfly);
     return build_schedule(p, cfg, out);
+}
+
+// Conventional BP set-up: node coordinates of every tile slot and the sensors on the device (once), and the
+// k-range of every (tile, sensor) row for this c0 (a kernel with the gather's own arithmetic; synchronises).
+pat_status ensure_onfly(pat_plan *p, float c0, void *stream, PatOnfly *out) {
+    const int64_t slots = p->dims.ntiles * kTilePix;
+    const int32_t S = p->dims.nsens;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!p->d_pix) {
+        std::vector<float> pix;
+        try { pix.assign((size_t)slots * 3, 0.0f); } catch (...) { return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
+        const int64_t n0 = p->grid.n[0], n1 = p->grid.n[1];
+        const float h = p->grid.h;
+        for (int64_t sl = 0; sl < slots; ++sl) {
+            int32_t pos = p->host_perm[(size_t)sl];
+            if (pos < 0) pos = p->host_perm[(size_t)(sl / kTilePix * kTilePix)];      // padding: the tile's first pixel
+            const int64_t q = p->roi.empty() ? pos : p->roi[(size_t)pos];
+            const int64_t id[3] = {q % n0, (q / n0) % n1, q / (n0 * n1)};
+            for (int dd = 0; dd < 3; ++dd) {
+                volatile float stepv = (float)id[dd] * h;                            // two roundings, no contraction
+                pix[(size_t)dd * slots + sl] = dd < p->grid.ndim ? p->grid.origin[dd] + stepv : 0.0f;
+            }
+        }
+        cudaError_t e = cudaMalloc((void **)&p->d_pix, pix.size() * sizeof(float));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&p->d_sens, (size_t)S * 3 * sizeof(float));
+        if (e == cudaSuccess) e = cudaMemcpy(p->d_pix, pix.data(), pix.size() * sizeof(float), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(p->d_sens, p->sensors.data(), (size_t)S * 3 * sizeof(float), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) {
+            cudaFree(p->d_pix); cudaFree(p->d_sens);
+            p->d_pix = p->d_sens = nullptr;
+            return cuda_fail(p, e, "conventional BP geometry upload");
+        }
+    }
+    out->pix = p->d_pix; out->sens = p->d_sens; out->pix_stride = slots;
+    out->inv_c0 = 1.0f / c0; out->t0 = p->t0; out->fs = p->fs; out->ndim = p->grid.ndim;
+    if (p->onfly_c0 != c0 || p->onfly_meta.empty()) {
+        const int64_t nrows = p->dims.ntiles * S;
+        void *d_meta = nullptr;
+        cudaError_t e = cudaMalloc(&d_meta, (size_t)nrows * 8);
+        if (e != cudaSuccess) return cuda_fail(p, e, "conventional BP row ranges");
+        PatLaunchCtx ctx{stream, p->num_sms, false};
+        int le = pat_launch_onfly_meta(ctx, *out, S, d_meta, nrows, p->dims.nt);
+        ++p->launches;
+        try { p->onfly_meta.resize((size_t)nrows * 2); } catch (...) { cudaFree(d_meta); return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
+        if (!le) e = cudaMemcpyAsync(p->onfly_meta.data(), d_meta, (size_t)nrows * 8, cudaMemcpyDeviceToHost, st);
+        if (!le && e == cudaSuccess) e = cudaStreamSynchronize(st);
+        cudaFree(d_meta);
+        if (le || e != cudaSuccess) { p->onfly_meta.clear(); return cuda_fail(p, le ? le : (int)e, "conventional BP row ranges"); }
+        p->onfly_c0 = c0;
+        // work lists of the previous c0 are stale
+        for (size_t q = 0; q < p->schedules.size();) {
+            if (p->schedules[q].cfg.onfly) {
+                if (p->schedules[q].d_sched) cudaFree(p->schedules[q].d_sched);
+                if (p->schedules[q].d_cta_chunk) cudaFree(p->schedules[q].d_cta_chunk);
+                p->schedules.erase(p->schedules.begin() + (long)q);
+            } else {
+                ++q;
+            }
+        }
+    }
+    return PAT_OK;
 }
 
 }  // namespace
@@ -398,6 +460,7 @@ extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, cons
     }
     p->device = dev;
     p->num_sms = sms;
+    p->host_perm = perm;
     e = cudaMemcpy(p->ws + p->lay.perm, perm.data(), perm.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { delete p; return cuda_fail(nullptr, e, "upload of the pixel permutation"); }
     if (!(std::getenv("PAT_NO_PIPE") && std::getenv("PAT_NO_PIPE")[0] == '1')) {
@@ -460,14 +523,30 @@ extern "C" pat_status pat_set_travel_times(pat_plan *p, const float *tau, int32_
     return PAT_OK;
 }
 
+static pat_status backproject_impl(pat_plan *p, const float *traces, float *images, int32_t nframes, void *stream,
+                                   bool conventional, float c0);
+
 extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *images,
                                       int32_t nframes, void *stream) {
+    return backproject_impl(p, traces, images, nframes, stream, false, 0.0f);
+}
+
+extern "C" pat_status pat_backproject_conventional(pat_plan *p, const float *traces, float *images,
+                                                   int32_t nframes, float c0, void *stream) {
+    if (!p) return PAT_ERR_INVALID_ARG;
+    if (!(c0 > 0.0f) || !std::isfinite(c0)) return fail(p, PAT_ERR_INVALID_ARG, "c0 must be finite and > 0");
+    if (p->sensors.empty()) return fail(p, PAT_ERR_BAD_STATE, "plan was created without sensor_xyz");
+    return backproject_impl(p, traces, images, nframes, stream, true, c0);
+}
+
+static pat_status backproject_impl(pat_plan *p, const float *traces, float *images, int32_t nframes, void *stream,
+                                   bool conventional, float c0) {
     if (!p) return PAT_ERR_INVALID_ARG;
     if (nframes < 0 || nframes > p->dims.max_batch)
         return fail(p, PAT_ERR_INVALID_ARG, "nframes outside [0, max_batch]");
     if (nframes == 0) return PAT_OK;
     if (!traces || !images) return fail(p, PAT_ERR_INVALID_ARG, "traces or images is NULL");
-    if (p->rows_set != p->dims.nsens)
+    if (!conventional && p->rows_set != p->dims.nsens)
         return fail(p, PAT_ERR_BAD_STATE, "pat_backproject before every tau row was set");
     const int td = is_device_ptr(traces), id = is_device_ptr(images);
     if (td < 0 || id < 0) return fail(p, PAT_ERR_CUDA, "cudaPointerGetAttributes failed");
@@ -505,8 +584,13 @@ extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *i
     }
     const int bp = pat_frames_per_group(nframes);
     PatSchedule *sc = nullptr;
-    {   // first use of this frame-count class after the table changed: builds the work list (synchronous)
-        pat_status ss = get_schedule(p, bp, &sc);
+    PatOnfly onfly;
+    {   // first use of this frame-count class after the table (or c0) changed: builds the work list (synchronous)
+        if (conventional) {
+            pat_status os = ensure_onfly(p, c0, stream, &onfly);
+            if (os != PAT_OK) return os;
+        }
+        pat_status ss = get_schedule(p, bp, conventional, &sc);
         if (ss != PAT_OK) return ss;
     }
     const bool prof = p->profiling == 1 && p->prof_events.size() < 3u * 65536u;
@@ -546,7 +630,8 @@ extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *i
         }
         e = pat_launch_gather(ctx, sc->cfg, (const float *)(p->ws + p->lay.tau), bw, sc->d_sched, sc->d_cta_chunk,
                               sc->grid_x, (const int32_t *)(p->ws + p->lay.perm), d_img, d.nsens, d.npix, d.nt,
-                              p->nt4, nframes, p->trace_ctas == sc->grid_x ? p->trace_dev : nullptr);
+                              p->nt4, nframes, p->trace_ctas == sc->grid_x ? p->trace_dev : nullptr,
+                              conventional ? &onfly : nullptr);
         if (e) return cuda_fail(p, e, "gather launch");
         ++p->launches;
     }
@@ -575,6 +660,8 @@ extern "C" pat_status pat_destroy(pat_plan *p) {
     }
     if (p) {
         drop_events(p); drop_schedules(p);
+        if (p->d_pix) cudaFree(p->d_pix);
+        if (p->d_sens) cudaFree(p->d_sens);
         if (p->copy_stream) { cudaStreamSynchronize((cudaStream_t)p->copy_stream); cudaStreamDestroy((cudaStream_t)p->copy_stream); }
         for (int q = 0; q < 2; ++q) {
             if (p->ev_h2d[q]) cudaEventDestroy((cudaEvent_t)p->ev_h2d[q]);

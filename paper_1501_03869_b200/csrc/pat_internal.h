@@ -47,6 +47,16 @@ struct PatGatherConfig {
     int R = 0;                // slots per stage
     int stages = 0;
     uint32_t hdr_bytes = 0, stage_bytes = 0;
+    bool onfly = false;       // work list of the conventional BP (k-ranges from the geometry, no table)
+};
+
+// Conventional BP: tau = |r - s| / c0 computed inside the gather.
+struct PatOnfly {
+    const float *pix = nullptr;     // device [3][pix_stride] node coordinates per tile slot
+    const float *sens = nullptr;    // device [nsens][3]
+    int64_t pix_stride = 0;
+    float inv_c0 = 0, t0 = 0, fs = 0;
+    int32_t ndim = 2;
 };
 
 // Host-built work list of one PatGatherConfig (built lazily, library-owned device memory).
@@ -87,6 +97,11 @@ struct pat_plan {
     void *copy_stream = nullptr;
     void *ev_h2d[2] = {nullptr, nullptr}, *ev_read[2] = {nullptr, nullptr};
     uint64_t host_calls = 0;
+    // conventional BP (pat_backproject_conventional): geometry on the device, k-ranges for the current c0
+    std::vector<int32_t> host_perm;   // tile slot -> ROI position (-1 = padding)
+    float *d_pix = nullptr, *d_sens = nullptr;
+    float onfly_c0 = 0;
+    std::vector<int32_t> onfly_meta;
     int profiling = 0;        // pat_set_profiling mode
     std::vector<void *> prof_events;  // cudaEvent_t triples: before pre-pass, between, after gather
     std::string err;
@@ -123,12 +138,14 @@ int pat_launch_stream_probe(const PatLaunchCtx &ctx, const void *a, int64_t a_by
 int pat_frames_per_group(int32_t nframes);
 bool pat_gather_blocked(int bp);       // trace layout [sensor][n/32][frame][32] instead of [sensor][n][frame]
 int pat_gather_wrmax(int bp);          // default / largest slot window for this frame-count class
-PatGatherConfig pat_gather_config(int bp, int wr, int R, int stages);   // 0 = choose automatically
+PatGatherConfig pat_gather_config(int bp, int wr, int R, int stages, bool onfly = false);   // 0 = choose automatically
 size_t pat_gather_smem_bytes(const PatGatherConfig &c);
 int pat_gather_occupancy(const PatGatherConfig &c, int *per_sm);
 int pat_launch_gather(const PatLaunchCtx &ctx, const PatGatherConfig &c, const float *u_t, const float *b,
                       const void *sched, const int32_t *cta_chunk, int grid_x, const int32_t *perm,
                       float *images, int32_t nsens, int64_t npix, int32_t nt, int32_t nt4, int32_t nframes,
-                      unsigned long long *trace = nullptr);   // trace: per-CTA timeline, 8 x u64 per CTA, or NULL
+                      unsigned long long *trace = nullptr,    // trace: per-CTA timeline, 8 x u64 per CTA, or NULL
+                      const PatOnfly *onfly = nullptr);       // conventional BP: u computed in the kernel
+int pat_launch_onfly_meta(const PatLaunchCtx &ctx, const PatOnfly &o, int32_t nsens, void *meta, int64_t nrows, int32_t nt);
 
 #endif  // PAT_INTERNAL_H_

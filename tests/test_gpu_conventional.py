@@ -1,0 +1,113 @@
+"""the conventional back projection with the delays computed inside the gather
+(pat_backproject_conventional) against the oracle: oracle.tau_conventional (the analytic delays
+in the fixed fp32 order) fed to oracle.backproject (Eq. 7).  Same bar as the table path."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as W
+from _cases import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+
+def _plan(geom, max_batch, mode=1):
+    import paper_1501_03869_b200 as pat
+    return pat.Plan(geom.n, geom.h, geom.origin, geom.c_map, geom.sensors, geom.roi_index, geom.nt, geom.fs,
+                    geom.t0, weighting=mode, max_batch=max_batch)
+
+
+def _run(plan, traces, c0, npix):
+    import torch
+    B = traces.shape[0]
+    img = torch.full((B, npix), float("nan"), dtype=torch.float32, device="cuda")
+    plan.backproject_conventional(torch.from_numpy(np.ascontiguousarray(traces)).cuda(), img, c0, B)
+    torch.cuda.synchronize()
+    return img.cpu().numpy()
+
+
+@pytest.mark.parametrize("B,mode", [(1, 1), (2, 1), (5, 0), (16, 1), (33, 2)])
+def test_conventional_2d_every_frame_class(B, mode):
+    geom = W.make_geometry(0)
+    c0 = 1560.0
+    rng = np.random.default_rng(100 + B)
+    traces = rng.standard_normal((B, geom.nsens, geom.nt)).astype(np.float32)
+    tau = oracle.tau_conventional(geom.n, geom.h, geom.origin, geom.sensors, geom.roi_index, c0)
+    ref = oracle.backproject(tau, traces, geom.fs, geom.t0, mode)
+    plan = _plan(geom, B, mode)
+    try:
+        got = _run(plan, traces, c0, geom.npix)
+    finally:
+        plan.close()
+    assert_parity(got, ref, "conventional B=%d mode=%d" % (B, mode))
+
+
+def test_conventional_3d_and_c0_change_and_mixing_with_the_table():
+    """3-D geometry; a second c0 on the same plan (work lists rebuilt); table calls in between are untouched."""
+    import torch
+    geom = W.make_geometry(3, True)
+    rng = np.random.default_rng(7)
+    traces = rng.standard_normal((3, geom.nsens, geom.nt)).astype(np.float32)
+    plan = _plan(geom, 3)
+    try:
+        for c0 in (1560.0, 1480.0):
+            tau = oracle.tau_conventional(geom.n, geom.h, geom.origin, geom.sensors, geom.roi_index, c0)
+            ref = oracle.backproject(tau, traces, geom.fs, geom.t0, 1)
+            assert_parity(_run(plan, traces, c0, geom.npix), ref, "3-D conventional c0=%g" % c0)
+        # the table path on the same plan, fed with the oracle's analytic table: the same image again
+        plan.set_travel_times(tau)
+        img = torch.empty((3, geom.npix), dtype=torch.float32, device="cuda")
+        plan.backproject(torch.from_numpy(traces).cuda(), img, 3)
+        torch.cuda.synchronize()
+        assert_parity(img.cpu().numpy(), ref, "table path with the analytic table")
+        assert_parity(_run(plan, traces, 1480.0, geom.npix), ref, "conventional after a table call")
+    finally:
+        plan.close()
+
+
+def test_conventional_windows_clipped_by_the_trace_ends():
+    """A short trace: many pixels fall before sample 0 or after nt-2 for some sensors (rows that are partly or
+    wholly invalid, long k-ranges) -- the index rule is the table path's."""
+    geom = W.make_geometry(0)
+    geom.nt = 96
+    rng = np.random.default_rng(3)
+    traces = rng.standard_normal((2, geom.nsens, geom.nt)).astype(np.float32)
+    c0 = 1500.0
+    tau = oracle.tau_conventional(geom.n, geom.h, geom.origin, geom.sensors, geom.roi_index, c0)
+    u = (tau.astype(np.float32) - np.float32(geom.t0)) * np.float32(geom.fs)
+    valid = (u >= 0) & (u < geom.nt - 1)
+    assert 0.02 < valid.mean() < 0.98                                # the case really is mixed
+    ref = oracle.backproject(tau, traces, geom.fs, geom.t0, 1)
+    plan = _plan(geom, 2)
+    try:
+        got = _run(plan, traces, c0, geom.npix)
+    finally:
+        plan.close()
+    assert_parity(got, ref, "clipped windows")
+
+
+def test_conventional_errors():
+    import torch
+    import paper_1501_03869_b200 as pat
+    geom = W.make_geometry(0)
+    plan = _plan(geom, 1)
+    tr = torch.zeros((1, geom.nsens, geom.nt), dtype=torch.float32, device="cuda")
+    img = torch.zeros((1, geom.npix), dtype=torch.float32, device="cuda")
+    try:
+        for bad in (0.0, -1.0, float("nan"), float("inf")):
+            with pytest.raises(pat.PatError) as ei:
+                plan.backproject_conventional(tr, img, bad, 1)
+            assert ei.value.status == pat.PAT_ERR_INVALID_ARG
+        with pytest.raises(pat.PatError) as ei:
+            plan.backproject_conventional(tr, img, 1500.0, 2)        # nframes > max_batch
+        assert ei.value.status == pat.PAT_ERR_INVALID_ARG
+    finally:
+        plan.close()
+    bare = pat.Plan(geom.n, geom.h, geom.origin, None, None, geom.roi_index, geom.nt, geom.fs, geom.t0, max_batch=1,
+                    nsens=geom.nsens)
+    try:
+        with pytest.raises(pat.PatError) as ei:
+            bare.backproject_conventional(tr, img, 1500.0, 1)
+        assert ei.value.status == pat.PAT_ERR_BAD_STATE
+    finally:
+        bare.close()
