@@ -61,6 +61,8 @@ def parse_args():
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--probe", default="", choices=["", "conventional", "eikonal"],
+                    help="run only this side probe on the config's geometry and print its JSON (ncu captures)")
     ap.add_argument("--tuning", type=str, default="", help="wr,rows,stages for pat_set_gather_tuning (0 = automatic)")
     return ap.parse_args()
 
@@ -467,6 +469,13 @@ def run_ours(args):
 
     k = args.config
     geom0 = W.make_geometry(k, args.reduced)
+    if args.probe:                                       # SURVEY.md 8(f) rows, off the headline path
+        if args.probe == "eikonal":
+            print(json.dumps({"offline_eikonal": eikonal_probe(geom0)}))
+        else:
+            g1, _, tr1 = prepare_inputs(k, args.reduced, 1)
+            print(json.dumps({"conventional_bp": conventional_probe(g1, tr1, batches=(args.batch or 1,))}))
+        return 0
     B = args.batch or geom0.batch
     do_sweep = (not args.no_sweep) and world == 1 and k in (1, 2) and not args.batch
     nframes = 64 if do_sweep else max(B, 16 if (world == 1 and not args.no_cpu_baseline) else B)

@@ -19,6 +19,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
+#include <cstdlib>
 #include <limits>
 #include <vector>
 
@@ -213,6 +214,7 @@ extern "C" pat_status pat_eikonal_travel_times_device(const pat_grid *grid, cons
     int64_t slots = std::min<int64_t>(count, (int64_t)sms * per_sm);
     const int64_t mem_cap = (int64_t)(free_b / 2) / (P.N * 8);
     slots = std::max<int64_t>(1, std::min(slots, mem_cap));
+    if (const char *ev = std::getenv("PAT_EIK_SLOTS")) slots = std::max<int64_t>(1, std::min<int64_t>(slots, std::atoi(ev)));
 
     cudaStream_t st = (cudaStream_t)stream;
     double *d_sh = nullptr, *d_T = nullptr, *d_sv = nullptr;
