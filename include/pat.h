@@ -128,6 +128,15 @@ pat_status pat_backproject(pat_plan *plan, const float *traces, float *images,
 pat_status pat_backproject_conventional(pat_plan *plan, const float *traces, float *images,
                                         int32_t nframes, float c0, void *stream);
 
+/* pat_set_roi_mask -- PAPER.md:81: "a specific region of interest can be selected for reconstruction to
+ * further reduce the reconstruction time" -- without touching the uploaded table.
+ *   mask   HOST uint8 [npix] in roi_index order, non-zero = reconstruct; NULL = all pixels again.
+ * Subsequent pat_backproject / pat_backproject_conventional calls skip every 256-pixel tile that holds no
+ * selected pixel (its part of the table is not read at all) and write 0 to unselected pixels; selected
+ * pixels get exactly the values of an unmasked call.  Synchronises the device and drops the work lists
+ * (rebuilt at the next call). */
+pat_status pat_set_roi_mask(pat_plan *plan, const uint8_t *mask);
+
 /* Frees the host-side plan; never frees caller memory.  NULL is allowed. */
 pat_status pat_destroy(pat_plan *plan);
 

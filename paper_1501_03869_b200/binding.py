@@ -84,6 +84,8 @@ def lib():
     L.pat_fmm_travel_times.argtypes = [gp, vp, vp, i32, vp, i64, i32, i32, i32, vp, i32]
     L.pat_compute_travel_times.restype = ctypes.c_int
     L.pat_compute_travel_times.argtypes = [vp, i32, i32, vp]
+    L.pat_set_roi_mask.restype = ctypes.c_int
+    L.pat_set_roi_mask.argtypes = [vp, vp]
     L.pat_backproject_conventional.restype = ctypes.c_int
     L.pat_backproject_conventional.argtypes = [vp, vp, vp, i32, ctypes.c_float, vp]
     L.pat_eikonal_travel_times_device.restype = ctypes.c_int
@@ -158,6 +160,13 @@ def pat_backproject_conventional(plan, traces, images, nframes, c0, stream=None)
     """Eq. 7 with tau = |r - s| / c0 computed in the kernel."""
     return _check(plan, lib().pat_backproject_conventional(plan, _addr(traces), _addr(images), nframes,
                                                            float(c0), _stream(stream)))
+
+
+def pat_set_roi_mask(plan, mask):
+    """mask: host uint8 [npix] (non-zero = reconstruct) or None for all pixels."""
+    if mask is not None:
+        mask = np.ascontiguousarray(mask, dtype=np.uint8)
+    return _check(plan, lib().pat_set_roi_mask(plan, _addr(mask) if mask is not None else None))
 
 
 def pat_destroy(plan):
@@ -262,6 +271,9 @@ class Plan:
     def backproject_conventional(self, traces, images, c0, nframes=None, stream=None):
         nframes = int(traces.shape[0]) if nframes is None else nframes
         return pat_backproject_conventional(self.handle, traces, images, nframes, c0, stream)
+
+    def set_roi_mask(self, mask):
+        return pat_set_roi_mask(self.handle, mask)
 
     def launches(self):
         return pat_kernel_launches(self.handle)

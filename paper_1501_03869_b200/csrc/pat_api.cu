@@ -115,6 +115,7 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
     if ((int64_t)S * p->nt4 > (int64_t)INT32_MAX) return fail(p, PAT_ERR_UNSUPPORTED, "nsens*nt exceeds 2^31");
     int64_t V = 0;
     for (int64_t r = 0; r < ntiles * S; ++r) {
+        if (!p->tile_active.empty() && !p->tile_active[(size_t)(r / S)]) continue;
         const int32_t kmin = meta[2 * r], kmax = meta[2 * r + 1] < 0 ? -1 : (meta[2 * r + 1] & 0x3FFFFFFF);
         if (kmax >= kmin) V += (kmax + 1 - (kmin & amask) + step - 1) / step;
     }
@@ -176,6 +177,7 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
             cur.push_back(sl);
         };
         for (int64_t t = 0; t < ntiles; ++t) {
+            if (!p->tile_active.empty() && !p->tile_active[(size_t)t]) continue;   // pat_set_roi_mask
             rest.clear();
             // whole rows in sensor order (their u rows stay consecutive: one bulk copy per chunk) ...
             for (int32_t s = 0; s < S; ++s) {
@@ -629,7 +631,8 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
                 p->trace_dev = nullptr;
         }
         e = pat_launch_gather(ctx, sc->cfg, (const float *)(p->ws + p->lay.tau), bw, sc->d_sched, sc->d_cta_chunk,
-                              sc->grid_x, (const int32_t *)(p->ws + p->lay.perm), d_img, d.nsens, d.npix, d.nt,
+                              sc->grid_x, p->d_perm_masked ? p->d_perm_masked : (const int32_t *)(p->ws + p->lay.perm),
+                              d_img, d.nsens, d.npix, d.nt,
                               p->nt4, nframes, p->trace_ctas == sc->grid_x ? p->trace_dev : nullptr,
                               conventional ? &onfly : nullptr);
         if (e) return cuda_fail(p, e, "gather launch");
@@ -660,6 +663,7 @@ extern "C" pat_status pat_destroy(pat_plan *p) {
     }
     if (p) {
         drop_events(p); drop_schedules(p);
+        if (p->d_perm_masked) cudaFree(p->d_perm_masked);
         if (p->d_pix) cudaFree(p->d_pix);
         if (p->d_sens) cudaFree(p->d_sens);
         if (p->copy_stream) { cudaStreamSynchronize((cudaStream_t)p->copy_stream); cudaStreamDestroy((cudaStream_t)p->copy_stream); }
@@ -757,5 +761,36 @@ extern "C" pat_status pat_compute_travel_times_gpu(pat_plan *p, int32_t max_roun
         if (cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) return fail(p, PAT_ERR_CUDA, "synchronise");
     }
     if (rounds_out) *rounds_out = worst;
+    return PAT_OK;
+}
+
+extern "C" pat_status pat_set_roi_mask(pat_plan *p, const uint8_t *mask) {
+    if (!p) return PAT_ERR_INVALID_ARG;
+    cudaError_t e = cudaDeviceSynchronize();            // no launch may still read the old permutation / lists
+    if (e != cudaSuccess) return cuda_fail(p, e, "synchronise");
+    drop_schedules(p);
+    if (!mask) {
+        p->tile_active.clear();
+        if (p->d_perm_masked) { cudaFree(p->d_perm_masked); p->d_perm_masked = nullptr; }
+        return PAT_OK;
+    }
+    const int64_t slots = p->dims.ntiles * kTilePix;
+    std::vector<int32_t> perm;
+    try {
+        perm = p->host_perm;
+        p->tile_active.assign((size_t)p->dims.ntiles, 0);
+    } catch (...) { return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
+    for (int64_t sl = 0; sl < slots; ++sl) {
+        const int32_t pos = perm[(size_t)sl];
+        if (pos < 0) continue;
+        if (mask[pos]) p->tile_active[(size_t)(sl / kTilePix)] = 1;
+        else perm[(size_t)sl] = -1;
+    }
+    if (!p->d_perm_masked) {
+        e = cudaMalloc((void **)&p->d_perm_masked, (size_t)slots * sizeof(int32_t));
+        if (e != cudaSuccess) { p->d_perm_masked = nullptr; p->tile_active.clear(); return cuda_fail(p, e, "roi mask allocation"); }
+    }
+    e = cudaMemcpy(p->d_perm_masked, perm.data(), (size_t)slots * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return cuda_fail(p, e, "roi mask upload");
     return PAT_OK;
 }

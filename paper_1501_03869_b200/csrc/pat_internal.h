@@ -102,6 +102,9 @@ struct pat_plan {
     float *d_pix = nullptr, *d_sens = nullptr;
     float onfly_c0 = 0;
     std::vector<int32_t> onfly_meta;
+    // pat_set_roi_mask: tiles without a selected pixel leave the work lists; unselected pixels are not written
+    std::vector<uint8_t> tile_active;   // empty = everything
+    int32_t *d_perm_masked = nullptr;   // [ntiles*256] perm with the unselected pixels set to -1
     int profiling = 0;        // pat_set_profiling mode
     std::vector<void *> prof_events;  // cudaEvent_t triples: before pre-pass, between, after gather
     std::string err;

@@ -5,7 +5,7 @@ import pytest
 
 import oracle
 import workloads as W
-from _cases import assert_parity, gpu_backproject
+from _cases import assert_parity, case, errors, gpu_backproject
 
 pytestmark = pytest.mark.gpu
 FS = 20e6
@@ -236,3 +236,47 @@ def test_host_calls_back_to_back_overlap_copies_and_kernels():
             assert_parity(im.numpy(), ref, "back-to-back host call %d" % q)
     finally:
         plan.close()
+
+
+def test_roi_mask_selects_pixels_without_touching_the_table():
+    """a region of interest can be selected for reconstruction.  Selected pixels get the values
+    of the full reconstruction, the others 0; tiles without a selected pixel leave the work list (fewer
+    launches' worth of work, same table); NULL restores everything; the conventional BP obeys the same mask."""
+    import torch
+    import paper_1501_03869_b200 as pat
+    geom, tau = case(0)
+    rng = np.random.default_rng(33)
+    traces = rng.standard_normal((2, geom.nsens, geom.nt)).astype(np.float32)
+    ref = oracle.backproject(tau, traces, geom.fs, geom.t0, 1)
+    x = geom.roi_index % geom.n[0]
+    for mask in (x < geom.n[0] // 3, rng.random(geom.npix) < 0.01, np.zeros(geom.npix, bool)):
+        plan = pat.Plan(geom.n, geom.h, geom.origin, geom.c_map, geom.sensors, geom.roi_index, geom.nt, geom.fs,
+                        geom.t0, max_batch=2)
+        try:
+            plan.set_travel_times(tau)
+            d_tr = torch.from_numpy(traces).cuda()
+            img = torch.full((2, geom.npix), float("nan"), dtype=torch.float32, device="cuda")
+            plan.set_roi_mask(mask)
+            plan.backproject(d_tr, img, 2)
+            torch.cuda.synchronize()
+            got = img.cpu().numpy()
+            assert (got[:, ~mask] == 0).all()
+            if mask.any():
+                rel, mx, sc = errors(got[:, mask], ref[:, mask])
+                assert rel <= 1e-5 and mx <= 1e-4 * np.max(np.abs(ref)), (rel, mx)
+            c0 = 1540.0
+            cref = oracle.backproject(oracle.tau_conventional(geom.n, geom.h, geom.origin, geom.sensors,
+                                                              geom.roi_index, c0), traces, geom.fs, geom.t0, 1)
+            plan.backproject_conventional(d_tr, img, c0, 2)
+            torch.cuda.synchronize()
+            got = img.cpu().numpy()
+            assert (got[:, ~mask] == 0).all()
+            if mask.any():
+                rel, mx, sc = errors(got[:, mask], cref[:, mask])
+                assert rel <= 1e-5 and mx <= 1e-4 * np.max(np.abs(cref)), (rel, mx)
+            plan.set_roi_mask(None)
+            plan.backproject(d_tr, img, 2)
+            torch.cuda.synchronize()
+            assert_parity(img.cpu().numpy(), ref, "mask removed")
+        finally:
+            plan.close()
