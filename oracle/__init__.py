@@ -15,7 +15,10 @@ from .build import build as _build
 _lib = None
 
 # (wp, wd) of  b = wp*p - wd*t*dp/dt  (Eq. 7; reading R1)
-WEIGHTS = {0: (1.0, 0.0), 1: (1.0, 1.0), 2: (2.0, 2.0)}
+# modes 3, 4: the same weights with p and dp/dt each interpolated AT t_ij and t = t_ij (Eq. 7 read
+# literally; R4b) -> oracle_backproject_exact
+WEIGHTS = {0: (1.0, 0.0), 1: (1.0, 1.0), 2: (2.0, 2.0), 3: (1.0, 1.0), 4: (2.0, 2.0)}
+EXACT_TIME_MODES = (3, 4)
 
 
 def lib():
@@ -34,6 +37,8 @@ def lib():
         L.oracle_weight.argtypes = [vp, i32, f64, f64, f64, vp]
         L.oracle_backproject.restype = ctypes.c_int
         L.oracle_backproject.argtypes = [vp, i64, vp, i32, i64, i32, i32, f32, f32, f64, f64, vp]
+        L.oracle_backproject_exact.restype = ctypes.c_int
+        L.oracle_backproject_exact.argtypes = L.oracle_backproject.argtypes
         _lib = L
     return _lib
 
@@ -115,7 +120,8 @@ def backproject(tau, traces, fs, t0=0.0, mode=1):
     pitch = tau.strides[0] // 4 if S > 1 else P
     img = np.zeros((B, P), dtype=np.float64)
     wp, wd = WEIGHTS[mode]
-    rc = lib().oracle_backproject(_p(tau), pitch, _p(traces), S, P, Nt, B,
+    fn = lib().oracle_backproject_exact if mode in EXACT_TIME_MODES else lib().oracle_backproject
+    rc = fn(_p(tau), pitch, _p(traces), S, P, Nt, B,
                                   float(np.float32(fs)), float(np.float32(t0)), wp, wd, _p(img))
     if rc:
         raise ValueError("oracle_backproject failed with code %d" % rc)

@@ -9,6 +9,7 @@
  *   oracle_weight       the integrand of Eq. 7 at the sample times
  *   oracle_backproject  Eq. 7 as a plain triple loop, PAPER.md:64-69 (Sec. II.C)
  *   oracle_tau_conventional  the conventional BP's analytic delays
+ *   oracle_backproject_exact Eq. 7 with the weight taken AT t_ij (its literal form)
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
  * reference legs may call this file.  It shares no code, header, table or
@@ -381,5 +382,55 @@ int oracle_backproject(const float *tau, int64_t tau_pitch, const float *traces,
         }
     }
     free(b);
+    return 0;
+}
+
+/* oracle_backproject_exact: Eq. 7 read literally ("p_i(t_ij) - t_ij * dp_i(t_ij)/dt"): the
+ * pressure AND its derivative are each sampled at the arrival time t_ij by linear interpolation, and the
+ * factor t is t_ij itself, not the sample times (reading R4b):
+ *     image[f][j] = sum_i  wp * [(1-a)*p[k] + a*p[k+1]]  -  wd * (u + t0*fs) * [(1-a)*D[k] + a*D[k+1]]
+ * with u, k, a exactly as in oracle_backproject (t_ij*fs = u + t0*fs in sample units; dp/dt = D*fs, so
+ * fs cancels) and D the finite difference of oracle_weight (central, one-sided at the two ends).
+ * Same arguments and return codes as oracle_backproject. */
+int oracle_backproject_exact(const float *tau, int64_t tau_pitch, const float *traces,
+                             int32_t nsens, int64_t npix, int32_t nt, int32_t nframes,
+                             float fs, float t0, double wp, double wd, double *image)
+{
+    if (nsens < 0 || npix < 0 || nt < 2 || nframes < 0 || tau_pitch < npix) return 1;
+    double *D = (double *)malloc((size_t)(nsens > 0 ? nsens : 1) * (size_t)nt * sizeof(double));
+    if (!D) return 2;
+    const double t0fs = (double)t0 * (double)fs;
+    const float ulim = (float)(nt - 1);
+    for (int32_t f = 0; f < nframes; ++f) {
+        const float *pf = traces + (int64_t)f * nsens * nt;
+        for (int32_t i = 0; i < nsens; ++i) {
+            const float *p = pf + (int64_t)i * nt;
+            double *Di = D + (int64_t)i * nt;
+            for (int32_t k = 0; k < nt; ++k) {
+                if (k == 0)            Di[k] = (double)p[1] - (double)p[0];
+                else if (k == nt - 1)  Di[k] = (double)p[nt - 1] - (double)p[nt - 2];
+                else                   Di[k] = ((double)p[k + 1] - (double)p[k - 1]) / 2.0;
+            }
+        }
+        #pragma omp parallel for schedule(static)
+        for (int64_t j = 0; j < npix; ++j) {
+            double acc = 0.0;
+            for (int32_t i = 0; i < nsens; ++i) {
+                float ts = tau[(int64_t)i * tau_pitch + j] - t0;   /* fp32 subtract */
+                float u = ts * fs;                                 /* ONE fp32 multiply */
+                if (!(u >= 0.0f && u < ulim)) continue;
+                float kf = floorf(u);
+                int32_t k = (int32_t)kf;
+                double a = (double)(u - kf);                       /* exact in fp32 */
+                const float *p = pf + (int64_t)i * nt;
+                const double *Di = D + (int64_t)i * nt;
+                double pv = (1.0 - a) * (double)p[k] + a * (double)p[k + 1];
+                double dv = (1.0 - a) * Di[k] + a * Di[k + 1];
+                acc += wp * pv - wd * ((double)u + t0fs) * dv;
+            }
+            image[(int64_t)f * npix + j] = acc;
+        }
+    }
+    free(D);
     return 0;
 }

@@ -276,3 +276,91 @@ def test_conventional_bp_point_source_focuses_at_the_source():
     img = oracle.backproject(tau, tr, fs, 0.0, 0)                               # plain delay and sum
     j = int(np.argmax(img[0]))
     assert (j % 31, j // 31) == src
+
+
+# ---- P16: Eq. 7 with the weight taken AT t_ij (modes 3, 4; oracle_backproject_exact) ----
+def _brute_exact(tau, tr, fs, t0, wp, wd):
+    """Independent pure-Python float64 loops: p and dp/dt each interpolated at t_ij, multiplied by t_ij*fs."""
+    B, S, Nt = tr.shape
+    P = tau.shape[1]
+    img = np.zeros((B, P))
+    for f in range(B):
+        for j in range(P):
+            acc = 0.0
+            for i in range(S):
+                u = (np.float32(tau[i, j]) - np.float32(t0)) * np.float32(fs)   # two fp32 roundings (R8)
+                if not (u >= 0 and u < Nt - 1):
+                    continue
+                k = int(np.floor(u))
+                a = float(u) - k
+                p = tr[f, i].astype(np.float64)
+
+                def D(n):
+                    if n == 0:
+                        return p[1] - p[0]
+                    if n == Nt - 1:
+                        return p[Nt - 1] - p[Nt - 2]
+                    return (p[n + 1] - p[n - 1]) / 2
+
+                t_samples = float(u) + float(np.float32(t0)) * float(np.float32(fs))
+                acc += wp * ((1 - a) * p[k] + a * p[k + 1]) - wd * t_samples * ((1 - a) * D(k) + a * D(k + 1))
+            img[f, j] = acc
+    return img
+
+
+@pytest.mark.parametrize("mode,t0", [(3, 0.0), (4, 0.0), (3, 3.25 / FS)])
+def test_p16_exact_time_brute_force(mode, t0):
+    rng = np.random.default_rng(16)
+    tau, tr = _rand_case(rng, S=4, P=64, Nt=32, B=2, umax=33)
+    tau[0, :5] = (np.array([0.0, 30.0, 30.999, 31.0, 0.25]) / FS).astype(np.float32)
+    tau = (tau + np.float32(t0)).astype(np.float32)
+    wp, wd = oracle.WEIGHTS[mode]
+    got = oracle.backproject(tau, tr, FS, t0=t0, mode=mode)
+    np.testing.assert_allclose(got, _brute_exact(tau, tr, FS, t0, wp, wd), rtol=1e-12, atol=1e-12)
+
+
+def test_p16_exact_time_closed_forms():
+    """p = c0 + c1*n: p(t) - t*p'(t) = c0 for every t.  p = n^2: lerp(p) = k^2 + a(2k+1), lerp(D) = 2u away from
+    the ends, so the term is k^2 + a(2k+1) - 2u^2.  A dropped term, a wrong sign or t_n instead of t_ij fails."""
+    rng = np.random.default_rng(17)
+    S, P, Nt = 5, 40, 128
+    tau = (rng.uniform(1.0, Nt - 3.0, size=(S, P)) / FS).astype(np.float32)
+    n = np.arange(Nt, dtype=np.float64)
+    ramp = (3.0 + 0.5 * n).astype(np.float32)
+    img = oracle.backproject(tau, np.broadcast_to(ramp, (1, S, Nt)).copy(), FS, mode=3)
+    np.testing.assert_allclose(img[0], 3.0 * S, rtol=0, atol=1e-9)
+    quad = (n * n).astype(np.float32)                     # exact in fp32
+    img = oracle.backproject(tau, np.broadcast_to(quad, (1, S, Nt)).copy(), FS, mode=3)
+    u = _u(tau).astype(np.float64)
+    k = np.floor(u)
+    a = u - k
+    np.testing.assert_allclose(img[0], (k * k + a * (2 * k + 1) - 2 * u * u).sum(axis=0), rtol=1e-12)
+
+
+def test_p16_exact_time_differs_from_sample_time_by_the_second_order_term():
+    """exact - sample-time = wd * a(1-a) * (D[k+1] - D[k]) per term (t0 = 0); mode 4 = 2 x mode 3."""
+    rng = np.random.default_rng(18)
+    tau, tr = _rand_case(rng, S=7, P=90, Nt=96, B=3)
+    u = _u(tau).astype(np.float64)
+    k = np.floor(u).astype(np.int64)
+    a = u - k
+    for mode_s, mode_e, wd in ((1, 3, 1.0), (2, 4, 2.0)):
+        base = oracle.backproject(tau, tr, FS, mode=mode_s)
+        corr = np.zeros_like(base)
+        for f in range(tr.shape[0]):
+            p = tr[f].astype(np.float64)
+            D = np.empty_like(p)
+            D[:, 1:-1] = (p[:, 2:] - p[:, :-2]) / 2
+            D[:, 0] = p[:, 1] - p[:, 0]
+            D[:, -1] = p[:, -1] - p[:, -2]
+            rows = np.arange(p.shape[0])[:, None]
+            corr[f] = (wd * a * (1 - a) * (D[rows, k + 1] - D[rows, k])).sum(axis=0)
+        np.testing.assert_allclose(oracle.backproject(tau, tr, FS, mode=mode_e), base + corr, rtol=1e-11, atol=1e-11)
+    np.testing.assert_array_equal(oracle.backproject(tau, tr, FS, mode=4), 2 * oracle.backproject(tau, tr, FS, mode=3))
+
+
+def test_p16_exact_time_out_of_record_terms_vanish():
+    tau = (np.array([[-1.0, 0.0, 5.5, 62.999, 63.0, np.nan, np.inf]]) / FS).astype(np.float32)
+    tr = np.ones((1, 1, 64), dtype=np.float32)
+    img = oracle.backproject(tau, tr, FS, mode=3)
+    np.testing.assert_array_equal(img[0], [0, 1, 1, 1, 0, 0, 0])
