@@ -42,7 +42,15 @@ typedef enum {
 typedef enum {
     PAT_W_DELAY_SUM = 0,        /* p                         (plain delay-and-sum)          */
     PAT_W_PAPER = 1,            /* p - t*dp/dt               (Eq. 7 as printed) */
-    PAT_W_UBP = 2               /* 2p - 2t*dp/dt             (universal BP, ref. [5])        */
+    PAT_W_UBP = 2,              /* 2p - 2t*dp/dt             (universal BP, ref. [5])        */
+    /* Eq. 7 read literally ("p_i(t_ij) - t_ij * dp_i(t_ij)/dt"):
+     * p AND dp/dt are each interpolated at the arrival time and the factor t is t_ij itself,
+     *     term = wp*[(1-a)*p[k] + a*p[k+1]] - wd*(u + t0*fs)*[(1-a)*D[k] + a*D[k+1]],
+     * which differs from modes 1, 2 by wd*a(1-a)*(D[k+1] - D[k]) per term (second order in 1/fs).
+     * The pre-pass then writes TWO channels per frame (wp*p and -wd*D), so a frame occupies two
+     * frame slots of the plan: nframes <= max_batch/2. */
+    PAT_W_PAPER_EXACT = 3,      /* p(t_ij) - t_ij*dp/dt(t_ij)                                */
+    PAT_W_UBP_EXACT = 4         /* 2 x PAT_W_PAPER_EXACT                                     */
 } pat_weighting;
 
 /* Regular grid of the speed-of-sound map / FMM domain. */
@@ -111,8 +119,10 @@ pat_status pat_set_travel_times(pat_plan *plan, const float *tau, int32_t sensor
  * the transfer of one call runs under the kernels of the previous call; everything is complete when
  * `stream` is (the host traces must stay untouched until then).  Inside a stream capture, or with
  * PAT_NO_PIPE=1, the copy is simply enqueued on `stream`.
- * nframes = 0 is a no-op; nframes > max_batch -> PAT_ERR_INVALID_ARG; tau rows missing ->
- * PAT_ERR_BAD_STATE. */
+ * With PAT_W_PAPER_EXACT / PAT_W_UBP_EXACT the term is the one stated at pat_weighting (two channels per
+ * frame through the same kernels) and nframes <= max_batch/2.
+ * nframes = 0 is a no-op; nframes > max_batch (> max_batch/2 for the _EXACT weightings) ->
+ * PAT_ERR_INVALID_ARG; tau rows missing -> PAT_ERR_BAD_STATE. */
 pat_status pat_backproject(pat_plan *plan, const float *traces, float *images,
                            int32_t nframes, void *stream);
 

@@ -5,7 +5,7 @@ is a thin ctypes binding with the same entry-point names.  There is no CPU fallb
 import fails loudly if the library is missing, and every compute call needs a B200.
 """
 from .binding import (PAT_OK, PAT_ERR_INVALID_ARG, PAT_ERR_BAD_STATE, PAT_ERR_CUDA, PAT_ERR_NOMEM,
-                      PAT_ERR_UNSUPPORTED, PAT_W_DELAY_SUM, PAT_W_PAPER, PAT_W_UBP, PatError, PatGrid,
+                      PAT_ERR_UNSUPPORTED, PAT_W_DELAY_SUM, PAT_W_PAPER, PAT_W_PAPER_EXACT, PAT_W_UBP, PAT_W_UBP_EXACT, PatError, PatGrid,
                       lib, library_path, pat_plan_workspace_bytes, pat_plan_create,
                       pat_set_travel_times, pat_backproject, pat_destroy, pat_last_error,
                       pat_kernel_launches, pat_set_gather_tuning, pat_fmm_travel_times,

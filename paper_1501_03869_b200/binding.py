@@ -10,7 +10,7 @@ import os
 import numpy as np
 
 PAT_OK, PAT_ERR_INVALID_ARG, PAT_ERR_BAD_STATE, PAT_ERR_CUDA, PAT_ERR_NOMEM, PAT_ERR_UNSUPPORTED = range(6)
-PAT_W_DELAY_SUM, PAT_W_PAPER, PAT_W_UBP = 0, 1, 2
+PAT_W_DELAY_SUM, PAT_W_PAPER, PAT_W_UBP, PAT_W_PAPER_EXACT, PAT_W_UBP_EXACT = 0, 1, 2, 3, 4
 _STATUS = ["PAT_OK", "PAT_ERR_INVALID_ARG", "PAT_ERR_BAD_STATE", "PAT_ERR_CUDA", "PAT_ERR_NOMEM",
            "PAT_ERR_UNSUPPORTED"]
 

@@ -269,7 +269,7 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
 pat_status get_schedule(pat_plan *p, int bp, bool onfly, PatSchedule **out) {
     for (PatSchedule &sc : p->schedules)
         if (sc.cfg.bp == bp && sc.cfg.onfly == onfly) { *out = &sc; return PAT_OK; }
-    PatGatherConfig cfg = pat_gather_config(bp, p->tune_wr, p->tune_R, p->tune_stages, onfly);
+    PatGatherConfig cfg = pat_gather_config(bp, p->tune_wr, p->tune_R, p->tune_stages, onfly, p->exact);
     return build_schedule(p, cfg, out);
 }
 
@@ -379,7 +379,7 @@ extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, cons
         return fail(nullptr, PAT_ERR_INVALID_ARG, "bad sizes (ndim, n, h, nsens, npix, nt or max_batch)");
     if (!(fs > 0.0f) || !std::isfinite(fs) || !std::isfinite(t0))
         return fail(nullptr, PAT_ERR_INVALID_ARG, "fs must be finite and > 0, t0 finite");
-    if (weighting < 0 || weighting > 2) return fail(nullptr, PAT_ERR_INVALID_ARG, "unknown weighting");
+    if (weighting < 0 || weighting > PAT_W_UBP_EXACT) return fail(nullptr, PAT_ERR_INVALID_ARG, "unknown weighting");
     int64_t N = 1;
     for (int d = 0; d < grid->ndim; ++d) N *= grid->n[d];
     if (!roi_index && npix != N)
@@ -414,7 +414,8 @@ extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, cons
     if (grid->ndim == 2) { p->grid.n[2] = 1; p->grid.origin[2] = 0.0f; }
     p->fs = fs; p->t0 = t0; p->weighting = weighting;
     p->nt4 = (nt + 3) / 4 * 4;
-    p->wp = weighting == PAT_W_UBP ? 2.0f : 1.0f;
+    p->exact = weighting == PAT_W_PAPER_EXACT || weighting == PAT_W_UBP_EXACT;
+    p->wp = (weighting == PAT_W_UBP || weighting == PAT_W_UBP_EXACT) ? 2.0f : 1.0f;
     p->wd = weighting == PAT_W_DELAY_SUM ? 0.0f : p->wp;
     p->ws = (char *)workspace;
     const char *env = std::getenv("PAT_NO_PDL");
@@ -546,6 +547,9 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
     if (!p) return PAT_ERR_INVALID_ARG;
     if (nframes < 0 || nframes > p->dims.max_batch)
         return fail(p, PAT_ERR_INVALID_ARG, "nframes outside [0, max_batch]");
+    const int32_t nch = p->exact ? 2 * nframes : nframes;       // exact-time weightings: two channels per frame
+    if (nch > p->dims.max_batch)
+        return fail(p, PAT_ERR_INVALID_ARG, "the _EXACT weightings need nframes <= max_batch/2 (two channels per frame)");
     if (nframes == 0) return PAT_OK;
     if (!traces || !images) return fail(p, PAT_ERR_INVALID_ARG, "traces or images is NULL");
     if (!conventional && p->rows_set != p->dims.nsens)
@@ -584,7 +588,7 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
         if (e != cudaSuccess) return cuda_fail(p, e, "traces H2D copy");
         ++p->host_calls;
     }
-    const int bp = pat_frames_per_group(nframes);
+    const int bp = pat_frames_per_group(nch);
     PatSchedule *sc = nullptr;
     PatOnfly onfly;
     {   // first use of this frame-count class after the table (or c0) changed: builds the work list (synchronous)
@@ -611,13 +615,13 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
     int e = 0;
     if (p->profiling == 4) {          // measurement: the step's footprint (table + b in, images out) as a plain stream
         e = pat_launch_stream_probe(ctx, p->ws + p->lay.tau, (int64_t)d.ntiles * kTilePix * d.nsens * 4,
-                                    bw, (int64_t)nframes * d.nsens * p->nt4 * 4, d_img, (int64_t)nframes * d.npix);
+                                    bw, (int64_t)nch * d.nsens * p->nt4 * 4, d_img, (int64_t)nframes * d.npix);
         if (e) return cuda_fail(p, e, "stream probe launch");
         ++p->launches;
         return PAT_OK;
     }
     if (p->profiling != 2) {
-        e = pat_launch_prepass(ctx, d_tr, bw, d_img, d.nsens, d.nt, p->nt4, nframes, bp, d.npix, p->wp, p->wd, t0fs);
+        e = pat_launch_prepass(ctx, d_tr, bw, d_img, d.nsens, d.nt, p->nt4, nframes, bp, d.npix, p->wp, p->wd, t0fs, p->exact);
         if (e) return cuda_fail(p, e, "pre-pass launch");
         ++p->launches;
     }
@@ -634,7 +638,7 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
                               sc->grid_x, p->d_perm_masked ? p->d_perm_masked : (const int32_t *)(p->ws + p->lay.perm),
                               d_img, d.nsens, d.npix, d.nt,
                               p->nt4, nframes, p->trace_ctas == sc->grid_x ? p->trace_dev : nullptr,
-                              conventional ? &onfly : nullptr);
+                              conventional ? &onfly : nullptr, t0fs);
         if (e) return cuda_fail(p, e, "gather launch");
         ++p->launches;
     }

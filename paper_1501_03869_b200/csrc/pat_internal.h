@@ -48,6 +48,7 @@ struct PatGatherConfig {
     int stages = 0;
     uint32_t hdr_bytes = 0, stage_bytes = 0;
     bool onfly = false;       // work list of the conventional BP (k-ranges from the geometry, no table)
+    bool exact = false;       // PAT_W_*_EXACT: the bp "frames" are channel pairs {wp*p, -wd*D} of bp/2 frames
 };
 
 // Conventional BP: tau = |r - s| / c0 computed inside the gather.
@@ -76,6 +77,7 @@ struct pat_plan {
     int32_t nt4 = 0;
     int32_t weighting = 1;
     float wp = 1, wd = 1;
+    bool exact = false;       // PAT_W_PAPER_EXACT / PAT_W_UBP_EXACT: weight taken at t_ij, two channels per frame
     char *ws = nullptr;       // device workspace base (borrowed)
     int device = 0;
     int num_sms = 0;
@@ -129,9 +131,10 @@ int pat_launch_row_meta(const PatLaunchCtx &ctx, const float *u_t, void *meta, i
 //   traces[f][s][n] (fp32) -> b[((g*nsens + s)*nt4 + n)*bp + fl],  f = g*bp + fl; rows n >= nt and
 //   frames f >= nframes are zero.  Also zeroes images[nframes*npix] (the gather accumulates into it).
 // bp >= 4 writes the blocked layout b[((g*nsens + s)*ntb + n/32)*bp + fl][n%32] (ntb = ceil(nt/32)).
+// exact (PAT_W_*_EXACT): bp counts CHANNELS, frame f owns channels 2f = wp*p[n] and 2f+1 = -wd*D[n].
 int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, float *images,
                        int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp,
-                       int64_t npix, float wp, float wd, float t0fs);
+                       int64_t npix, float wp, float wd, float t0fs, bool exact = false);
 
 // Measurement only (pat_set_profiling mode 4): stream a_bytes + c_bytes in, nout floats out.
 int pat_launch_stream_probe(const PatLaunchCtx &ctx, const void *a, int64_t a_bytes, const void *c, int64_t c_bytes,
@@ -141,14 +144,15 @@ int pat_launch_stream_probe(const PatLaunchCtx &ctx, const void *a, int64_t a_by
 int pat_frames_per_group(int32_t nframes);
 bool pat_gather_blocked(int bp);       // trace layout [sensor][n/32][frame][32] instead of [sensor][n][frame]
 int pat_gather_wrmax(int bp);          // default / largest slot window for this frame-count class
-PatGatherConfig pat_gather_config(int bp, int wr, int R, int stages, bool onfly = false);   // 0 = choose automatically
+PatGatherConfig pat_gather_config(int bp, int wr, int R, int stages, bool onfly = false, bool exact = false);   // 0 = choose automatically
 size_t pat_gather_smem_bytes(const PatGatherConfig &c);
 int pat_gather_occupancy(const PatGatherConfig &c, int *per_sm);
 int pat_launch_gather(const PatLaunchCtx &ctx, const PatGatherConfig &c, const float *u_t, const float *b,
                       const void *sched, const int32_t *cta_chunk, int grid_x, const int32_t *perm,
                       float *images, int32_t nsens, int64_t npix, int32_t nt, int32_t nt4, int32_t nframes,
                       unsigned long long *trace = nullptr,    // trace: per-CTA timeline, 8 x u64 per CTA, or NULL
-                      const PatOnfly *onfly = nullptr);       // conventional BP: u computed in the kernel
+                      const PatOnfly *onfly = nullptr,        // conventional BP: u computed in the kernel
+                      float t0fs = 0.0f);                     // exact-time weightings: t0*fs
 int pat_launch_onfly_meta(const PatLaunchCtx &ctx, const PatOnfly &o, int32_t nsens, void *meta, int64_t nrows, int32_t nt);
 
 #endif  // PAT_INTERNAL_H_

@@ -232,6 +232,67 @@ prepass_small_kernel(const float *__restrict__ traces, float *__restrict__ b, fl
     }
 }
 
+// ---- exact-time weightings (PAT_W_*_EXACT; Eq. 7 read literally) ------------------------
+// The gather interpolates p AND dp/dt at t_ij, so the pre-pass writes two CHANNELS per frame in the layout
+// of the channel count bp: channel 2f = wp*p_f[n], channel 2f+1 = -wd*D_f[n] (D as in weight_at; both
+// products are exact for wp = wd in {1, 2}).  One thread per (frame, sensor, 4 consecutive samples).
+//   LAYOUT 0  bp = 2   [sensor][sample][2]: a thread's 4 samples are 32 contiguous bytes
+//   LAYOUT 1  bp = 4, 8, 16 blocked [sensor][n/32][channel][32]: one 16-byte store per channel
+//   LAYOUT 2  bp = 32  [sensor][sample][32]: the 16 frames of a group are the fastest thread index, so that a
+//             half-warp writes the 128-byte line of one sample
+template <int LAYOUT>
+__global__ void __launch_bounds__(256)
+prepass_exact_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
+                     int32_t nsens, int32_t nt, int32_t nt4, int32_t ntb, int32_t nframes, int32_t log2_bp,
+                     int64_t npix, float wp, float wd) {
+    asm volatile("griddepcontrol.launch_dependents;");
+    {
+        const int64_t nblk = (int64_t)gridDim.x * gridDim.y * gridDim.z;
+        const int64_t blk = ((int64_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+        const int64_t tot = npix * nframes;
+        if (blk * 256 < tot)
+            for (int64_t q = blk * 256 + threadIdx.x; q < tot; q += nblk * 256) images[q] = 0.0f;
+    }
+    const int32_t s = blockIdx.y, bp = 1 << log2_bp;
+    int32_t f, q;
+    if (LAYOUT == 2) { f = blockIdx.z * 16 + (threadIdx.x & 15); q = blockIdx.x * 16 + (threadIdx.x >> 4); }
+    else             { f = blockIdx.z; q = blockIdx.x * 256 + threadIdx.x; }
+    const int32_t quads = LAYOUT == 1 ? ntb * 8 : nt4 >> 2;
+    if (q >= quads) return;
+    const int32_t n0 = q << 2;
+    float pv[4] = {0.0f, 0.0f, 0.0f, 0.0f}, dv[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+    if (f < nframes && n0 < nt) {
+        float w[6];
+        load_quad(traces + ((int64_t)f * nsens + s) * nt, n0, nt, w);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int32_t n = n0 + j;
+            if (n < nt) {
+                const float pm = w[j], pn = w[j + 1], pp = w[j + 2];
+                float D;
+                if (n == 0)            D = __fsub_rn(pp, pn);
+                else if (n == nt - 1)  D = __fsub_rn(pn, pm);
+                else                   D = 0.5f * __fsub_rn(pp, pm);
+                pv[j] = wp * pn;
+                dv[j] = -wd * D;
+            }
+        }
+    }
+    const int32_t ch = 2 * f, g = ch >> log2_bp, cl = ch & (bp - 1);
+    if (LAYOUT == 1) {
+        float *dst = b + (((((int64_t)g * nsens + s) * ntb + (n0 >> 5)) << log2_bp) + cl) * 32 + (n0 & 31);
+        *reinterpret_cast<float4 *>(dst) = make_float4(pv[0], pv[1], pv[2], pv[3]);
+        *reinterpret_cast<float4 *>(dst + 32) = make_float4(dv[0], dv[1], dv[2], dv[3]);
+    } else if (LAYOUT == 0) {
+        float4 *dst = reinterpret_cast<float4 *>(b + (((int64_t)g * nsens + s) * nt4 + n0) * 2);
+        dst[0] = make_float4(pv[0], dv[0], pv[1], dv[1]);
+        dst[1] = make_float4(pv[2], dv[2], pv[3], dv[3]);
+    } else {
+        float *dst = b + ((((int64_t)g * nsens + s) * nt4 + n0) << log2_bp) + cl;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) *reinterpret_cast<float2 *>(dst + ((int64_t)j << log2_bp)) = make_float2(pv[j], dv[j]);
+    }
+}
 
 // ---- measurement only: the same bytes as one step, as a plain stream ----------------------------
 // Reads n16 16-byte words (the u table and b), writes nout floats (the images).  bench.py times it in the
@@ -285,7 +346,25 @@ int pat_launch_retile(const PatLaunchCtx &ctx, const float *src, float *u_t, con
 
 int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, float *images,
                        int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp,
-                       int64_t npix, float wp, float wd, float t0fs) {
+                       int64_t npix, float wp, float wd, float t0fs, bool exact) {
+    if (exact) {                                   // bp counts channels, two per frame
+        if (bp < 2 || bp > 32) return (int)cudaErrorInvalidValue;
+        int log2_bp = 0;
+        while ((1 << log2_bp) < bp) ++log2_bp;
+        const int32_t fpg = bp / 2, groups = (nframes + fpg - 1) / fpg, ntb = (nt + 31) / 32;
+        cudaStream_t st = (cudaStream_t)ctx.stream;
+        if (bp == 2) {
+            dim3 grid((unsigned)(((nt4 >> 2) + 255) / 256), (unsigned)nsens, (unsigned)groups);
+            prepass_exact_kernel<0><<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd);
+        } else if (pat_gather_blocked(bp)) {
+            dim3 grid((unsigned)((ntb * 8 + 255) / 256), (unsigned)nsens, (unsigned)(groups * fpg));
+            prepass_exact_kernel<1><<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd);
+        } else {
+            dim3 grid((unsigned)(((nt4 >> 2) + 15) / 16), (unsigned)nsens, (unsigned)groups);
+            prepass_exact_kernel<2><<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd);
+        }
+        return (int)cudaGetLastError();
+    }
     if (bp <= 2) {
         const int64_t work = (int64_t)nsens * (nt4 >> 2);
         int64_t blocks = (work + 255) / 256;

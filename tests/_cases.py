@@ -56,7 +56,7 @@ def gpu_backproject(geom, tau, traces, mode=1, max_batch=None, tuning=None, host
     import paper_1501_03869_b200 as pat
     B = traces.shape[0]
     plan = pat.Plan(geom.n, geom.h, geom.origin, geom.c_map, geom.sensors, geom.roi_index, geom.nt,
-                    geom.fs, geom.t0 if t0 is None else t0, weighting=mode, max_batch=max_batch or max(B, 1))
+                    geom.fs, geom.t0 if t0 is None else t0, weighting=mode, max_batch=max_batch or max(B, 1) * (2 if mode >= 3 else 1))   # _EXACT: two channels per frame
     try:
         if tuning:
             pat.pat_set_gather_tuning(plan.handle, *tuning)

@@ -68,7 +68,7 @@ def _create(**kw):
 
 
 @pytest.mark.parametrize("kw", [
-    dict(nsens=0), dict(nt=1), dict(fs=0.0), dict(fs=float("nan")), dict(weighting=3), dict(max_batch=0),
+    dict(nsens=0), dict(nt=1), dict(fs=0.0), dict(fs=float("nan")), dict(weighting=5), dict(max_batch=0),
     dict(roi_index=np.array([5, 5, 6], np.int64), npix=3), dict(roi_index=np.array([1, 4096], np.int64), npix=2),
     dict(roi_index=None, npix=100), dict(c_map=np.zeros(4096, np.float32)),
     dict(c_map=np.full(4096, np.inf, np.float32)), dict(workspace=None), dict(workspace=260),
