@@ -19,6 +19,7 @@ CPU FMM (input preparation, untimed).  Prints ONE JSON line (rank 0):
   cpu_baseline the oracle (oracle/pat_oracle.c) timed on this box's host cores, rank 0, N = 1.
   large_workload_probe  the same path on configs[4] reduced (537 MB table): the gather's steady-state rate.
   conventional_bp  PAPER.md:69's comparison method with the delays computed in the kernel (no table stream).
+  exact_time_weighting  Eq. 7 with p and dp/dt both taken at t_ij (PAT_W_PAPER_EXACT, two channels per frame).
   offline_eikonal  (not part of the step) the tau table of the geometry solved on the GPU vs the CPU fast marching.
   sweep        B = 1..64 on the same geometry (N = 1 only): ms/frame, GUpd/s, HBM fraction and the
                SM-side (shared-memory bandwidth) fraction, because for B >~ 4 the path is not
@@ -61,7 +62,7 @@ def parse_args():
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--probe", default="", choices=["", "conventional", "eikonal"],
+    ap.add_argument("--probe", default="", choices=["", "conventional", "eikonal", "exact"],
                     help="run only this side probe on the config's geometry and print its JSON (ncu captures)")
     ap.add_argument("--tuning", type=str, default="", help="wr,rows,stages for pat_set_gather_tuning (0 = automatic)")
     return ap.parse_args()
@@ -222,11 +223,31 @@ def conventional_probe(geom, traces, batches=(1, 32)):
     return out
 
 
+def exact_time_probe(geom, tau, traces, peak_gbs, batches=(1, 16), steps=400):
+    """Eq. 7 with p and dp/dt both interpolated at t_ij (PAT_W_PAPER_EXACT): the same
+    table stream, two trace channels per frame through the pre-pass and the gather.  Timed like the headline
+    (rotating plans so that the table comes from HBM, CUDA graph replay, events on the launching stream)."""
+    import paper_1501_03869_b200 as pat
+    out = []
+    for B in batches:
+        rig = Rig(geom, tau, traces, B, weighting=pat.PAT_W_PAPER_EXACT)
+        rig.run(rig.R)                                   # first calls build the work lists: outside the capture
+        rig.torch.cuda.synchronize()
+        rig.capture_round()
+        n = max(20, steps // B)
+        ms = time_steps(rig, n, 10) / n
+        rig.close()
+        upd = float(B) * geom.nsens * geom.npix
+        out.append({"B": B, "ms_per_frame": round(ms / B, 6), "gupd_s": round(upd / (ms * 1e-3) / 1e9, 1),
+                    "step_hbm_frac": round(algorithmic_bytes(geom.nsens, geom.npix, geom.nt, B) / (ms * 1e-3) / 1e9 / peak_gbs, 4)})
+    return out
+
+
 class Rig:
     """R rotating plans (own tau copy, traces, images) so that consecutive steps never find their
     tau table in L2: R * tau bytes > 3 x L2."""
 
-    def __init__(self, geom, tau, traces, B, variant=0, host=False):
+    def __init__(self, geom, tau, traces, B, variant=0, host=False, weighting=None):
         import torch
         import paper_1501_03869_b200 as pat
         self.pat, self.torch, self.geom, self.B = pat, torch, geom, B
@@ -241,7 +262,8 @@ class Rig:
         F = traces.shape[0]
         for r in range(self.R):
             p = pat.Plan(geom.n, geom.h, geom.origin, None, geom.sensors, geom.roi_index, geom.nt, geom.fs,
-                         geom.t0, weighting=pat.PAT_W_PAPER, max_batch=B)
+                         geom.t0, weighting=pat.PAT_W_PAPER if weighting is None else weighting,
+                         max_batch=B if weighting is None or weighting < pat.PAT_W_PAPER_EXACT else 2 * B)
             if variant:
                 pat.pat_set_gather_tuning(p.handle, *variant)
             p.set_travel_times(tau)
@@ -472,6 +494,9 @@ def run_ours(args):
     if args.probe:                                       # SURVEY.md 8(f) rows, off the headline path
         if args.probe == "eikonal":
             print(json.dumps({"offline_eikonal": eikonal_probe(geom0)}))
+        elif args.probe == "exact":
+            g1, tau1, tr1 = prepare_inputs(k, args.reduced, max(1, args.batch or 1))
+            print(json.dumps({"exact_time_weighting": exact_time_probe(g1, tau1, tr1, peak_gbs, batches=(args.batch or 1,))}))
         else:
             g1, _, tr1 = prepare_inputs(k, args.reduced, 1)
             print(json.dumps({"conventional_bp": conventional_probe(g1, tr1, batches=(args.batch or 1,))}))
@@ -513,10 +538,11 @@ def run_ours(args):
                  "ms_per_frame": round(m4["ms_per_frame"], 6), "gupd_s": round(m4["gupd_s"], 1),
                  "step_hbm_frac": round(m4["step_hbm_frac"], 4), "gather_hbm_frac": round(m4["gather_gbs"] / peak_gbs, 4),
                  "full_size_result": "profiles/r01_config4_full.md (34.4 GB table: 6.26 ms/frame, 0.84 of the HBM peak)"}
-    eik, conv = None, None
+    eik, conv, exact = None, None, None
     if do_sweep:
         eik = eikonal_probe(geom)
         conv = conventional_probe(geom, traces)
+        exact = exact_time_probe(geom, tau, traces, peak_gbs)
     sampler.stop_flag = True
     sampler.join(timeout=2.0)
     clocks_main = sampler.summary()
@@ -567,6 +593,8 @@ def run_ours(args):
         line["offline_eikonal"] = eik
     if conv:
         line["conventional_bp"] = conv
+    if exact:
+        line["exact_time_weighting"] = exact
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(geom, tau, traces)
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
