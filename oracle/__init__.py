@@ -37,6 +37,10 @@ def lib():
         L.oracle_weight.argtypes = [vp, i32, f64, f64, f64, vp]
         L.oracle_backproject.restype = ctypes.c_int
         L.oracle_backproject.argtypes = [vp, i64, vp, i32, i64, i32, i32, f32, f32, f64, f64, vp]
+        L.oracle_solid_angle_weights.restype = ctypes.c_int
+        L.oracle_solid_angle_weights.argtypes = [i32, vp, f32, vp, vp, vp, i32, vp, i64, vp, vp]
+        L.oracle_backproject_weighted.restype = ctypes.c_int
+        L.oracle_backproject_weighted.argtypes = [vp, vp, i64, vp, i32, i64, i32, i32, f32, f32, f64, f64, vp]
         L.oracle_backproject_exact.restype = ctypes.c_int
         L.oracle_backproject_exact.argtypes = L.oracle_backproject.argtypes
         _lib = L
@@ -107,9 +111,34 @@ def weight(p, mode=1, t0fs=0.0):
     return b
 
 
-def backproject(tau, traces, fs, t0=0.0, mode=1):
-    """Eq. 7 image, double [nframes][npix]; tau fp32 [nsens][npix], traces fp32 [B][S][Nt]."""
+def solid_angle_weights(n, h, origin, sensors, normals, roi_index, return_omega0=False):
+    """w[i][j] fp32 = dOmega_ij / Omega0_j of the universal BP [5] (R27)."""
+    ndim = len(n)
+    n3 = np.array(list(n) + [1] * (3 - ndim), dtype=np.int32)
+    org = np.array(list(origin) + [0.0] * (3 - len(origin)), dtype=np.float32)
+    sens = np.ascontiguousarray(sensors, dtype=np.float32).reshape(-1, 3)
+    nrm = np.ascontiguousarray(normals, dtype=np.float32).reshape(-1, 3)
+    assert nrm.shape == sens.shape
+    roi = None if roi_index is None else np.ascontiguousarray(roi_index, dtype=np.int64)
+    npix = int(np.prod(n3)) if roi is None else roi.size
+    w = np.empty((sens.shape[0], npix), dtype=np.float32)
+    om = np.empty(npix, dtype=np.float64)
+    rc = lib().oracle_solid_angle_weights(ndim, _p(n3), float(np.float32(h)), _p(org), _p(sens), _p(nrm),
+                                          sens.shape[0], _p(roi) if roi is not None else None, npix, _p(w), _p(om))
+    if rc:
+        raise ValueError("oracle_solid_angle_weights failed with code %d" % rc)
+    return (w, om) if return_omega0 else w
+
+
+def backproject(tau, traces, fs, t0=0.0, mode=1, weights=None):
+    """Eq. 7 image, double [nframes][npix]; tau fp32 [nsens][npix], traces fp32 [B][S][Nt].
+    weights: optional fp32 [nsens][npix] multiplying every term (modes 0-2 only)."""
     tau = np.asarray(tau)
+    if weights is not None:
+        assert mode in (0, 1, 2)
+        tau = np.ascontiguousarray(tau)
+        weights = np.ascontiguousarray(weights, dtype=np.float32)
+        assert weights.shape == tau.shape
     assert tau.dtype == np.float32 and tau.ndim == 2 and tau.strides[1] == 4
     traces = np.ascontiguousarray(traces, dtype=np.float32)
     if traces.ndim == 2:
@@ -120,6 +149,12 @@ def backproject(tau, traces, fs, t0=0.0, mode=1):
     pitch = tau.strides[0] // 4 if S > 1 else P
     img = np.zeros((B, P), dtype=np.float64)
     wp, wd = WEIGHTS[mode]
+    if weights is not None:
+        rc = lib().oracle_backproject_weighted(_p(tau), _p(weights), pitch, _p(traces), S, P, Nt, B,
+                                               float(np.float32(fs)), float(np.float32(t0)), wp, wd, _p(img))
+        if rc:
+            raise ValueError("oracle_backproject_weighted failed with code %d" % rc)
+        return img
     fn = lib().oracle_backproject_exact if mode in EXACT_TIME_MODES else lib().oracle_backproject
     rc = fn(_p(tau), pitch, _p(traces), S, P, Nt, B,
                                   float(np.float32(fs)), float(np.float32(t0)), wp, wd, _p(img))

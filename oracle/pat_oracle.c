@@ -10,6 +10,8 @@
  *   oracle_backproject  Eq. 7 as a plain triple loop, PAPER.md:64-69 (Sec. II.C)
  *   oracle_tau_conventional  the conventional BP's analytic delays
  *   oracle_backproject_exact Eq. 7 with the weight taken AT t_ij (its literal form)
+ *   oracle_solid_angle_weights, oracle_backproject_weighted  the "exact BP algorithm [5]" that Eq. 7
+ *                       approximates: every term weighted by dOmega_ij / Omega0_j
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
  * reference legs may call this file.  It shares no code, header, table or
@@ -432,5 +434,87 @@ int oracle_backproject_exact(const float *tau, int64_t tau_pitch, const float *t
         }
     }
     free(D);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------- */
+/* "Eq. 7 can be viewed as an approximation to the exact BP algorithm [5].  It assumes a
+ * circular scanning geometry and that the scanning radius is considerably larger than the region of
+ * interest."  Ref. [5] (universal back projection) weights the term of detector i at point r_j by the solid
+ * angle dOmega_ij the detector element subtends at r_j, normalised by the total Omega0_j:
+ *     P(r_j) = sum_i (dOmega_ij / Omega0_j) * b_i(t_ij),   b = 2p - 2t dp/dt  (weighting mode 2),
+ *     dOmega_ij = dS_i * n_i . (s_i - r_j) / |s_i - r_j|^3 ,   Omega0_j = sum_i dOmega_ij ,
+ * n_i = the unit normal of the detection surface at s_i pointing AWAY from the imaged region.  Equal element
+ * areas dS_i cancel.  Under the paper's assumption (large circle) dOmega_ij / Omega0_j -> 1/S and the sum
+ * becomes Eq. 7 up to the constant 1/S.  Readings (R27): in 2-D (ring of detectors in the image
+ * plane) the subtended ANGLE n.e/|e|^2 takes the place of the solid angle; a detector facing away from the
+ * point (n.e <= 0) or sitting on it (|e| = 0) gets weight 0; a point that no detector faces gets all-zero
+ * weights.  SURVEY.md 8(f) NEXT-4.
+ *
+ * oracle_solid_angle_weights: node coordinates x_d = origin_d + i_d*h and everything after in double from the
+ * fp32 inputs.  w: fp32 out [nsens][npix] (the normalised weights); omega0: double out [npix] or NULL (the
+ * un-normalised sum, for the closed-curve / closed-surface pins).  Returns 0, or 1 bad argument. */
+int oracle_solid_angle_weights(int32_t ndim, const int32_t *n, float h, const float *origin,
+                               const float *sensors, const float *normals, int32_t nsens,
+                               const int64_t *roi, int64_t npix, float *w, double *omega0)
+{
+    if ((ndim != 2 && ndim != 3) || !n || !origin || !sensors || !normals || !w || nsens < 0) return 1;
+    const int64_t n0 = n[0], n1 = n[1];
+    for (int64_t j = 0; j < npix; ++j) {
+        const int64_t q = roi ? roi[j] : j;
+        const int64_t id[3] = { q % n0, (q / n0) % n1, q / (n0 * n1) };
+        double r[3] = { 0.0, 0.0, 0.0 };
+        for (int d = 0; d < ndim; ++d) r[d] = (double)origin[d] + (double)id[d] * (double)h;
+        double total = 0.0;
+        for (int pass = 0; pass < 2; ++pass) {
+            for (int32_t i = 0; i < nsens; ++i) {
+                double dot = 0.0, d2 = 0.0;
+                for (int d = 0; d < ndim; ++d) {
+                    const double e = (double)sensors[3 * (int64_t)i + d] - r[d];
+                    dot += (double)normals[3 * (int64_t)i + d] * e;
+                    d2 += e * e;
+                }
+                double om = 0.0;
+                if (dot > 0.0 && d2 > 0.0) om = ndim == 3 ? dot / (d2 * sqrt(d2)) : dot / d2;
+                if (pass == 0) total += om;
+                else w[(int64_t)i * npix + j] = total > 0.0 ? (float)(om / total) : 0.0f;
+            }
+        }
+        if (omega0) omega0[j] = total;
+    }
+    return 0;
+}
+
+/* oracle_backproject_weighted: oracle_backproject with every term multiplied by wgt[i][j] (fp32, same pitch
+ * as tau):  image[f][j] = sum_i wgt_ij * [ (1-a)*b_fi[k] + a*b_fi[k+1] ].  Same arguments otherwise. */
+int oracle_backproject_weighted(const float *tau, const float *wgt, int64_t tau_pitch, const float *traces,
+                                int32_t nsens, int64_t npix, int32_t nt, int32_t nframes,
+                                float fs, float t0, double wp, double wd, double *image)
+{
+    if (nsens < 0 || npix < 0 || nt < 2 || nframes < 0 || tau_pitch < npix || !wgt) return 1;
+    double *b = (double *)malloc((size_t)(nsens > 0 ? nsens : 1) * (size_t)nt * sizeof(double));
+    if (!b) return 2;
+    const double t0fs = (double)t0 * (double)fs;
+    const float ulim = (float)(nt - 1);
+    for (int32_t f = 0; f < nframes; ++f) {
+        for (int32_t i = 0; i < nsens; ++i)
+            oracle_weight(traces + ((int64_t)f * nsens + i) * nt, nt, wp, wd, t0fs, b + (int64_t)i * nt);
+        #pragma omp parallel for schedule(static)
+        for (int64_t j = 0; j < npix; ++j) {
+            double acc = 0.0;
+            for (int32_t i = 0; i < nsens; ++i) {
+                float ts = tau[(int64_t)i * tau_pitch + j] - t0;   /* fp32 subtract */
+                float u = ts * fs;                                 /* ONE fp32 multiply */
+                if (!(u >= 0.0f && u < ulim)) continue;
+                float kf = floorf(u);
+                int32_t k = (int32_t)kf;
+                float a = u - kf;                                  /* exact in fp32 */
+                const double *bi = b + (int64_t)i * nt;
+                acc += (double)wgt[(int64_t)i * tau_pitch + j] * ((1.0 - (double)a) * bi[k] + (double)a * bi[k + 1]);
+            }
+            image[(int64_t)f * npix + j] = acc;
+        }
+    }
+    free(b);
     return 0;
 }

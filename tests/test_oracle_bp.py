@@ -364,3 +364,118 @@ def test_p16_exact_time_out_of_record_terms_vanish():
     tr = np.ones((1, 1, 64), dtype=np.float32)
     img = oracle.backproject(tau, tr, FS, mode=3)
     np.testing.assert_array_equal(img[0], [0, 1, 1, 1, 0, 0, 0])
+
+
+# ---- P17: solid-angle weights of the universal BP [5] and the weighted sum (R27) ----
+def _ring(S, R):
+    th = 2 * np.pi * np.arange(S) / S
+    s = np.stack([R * np.cos(th), R * np.sin(th), np.zeros(S)], axis=1)
+    nrm = np.stack([np.cos(th), np.sin(th), np.zeros(S)], axis=1)
+    return s.astype(np.float32), nrm.astype(np.float32)
+
+
+def test_p17_ring_subtends_two_pi_and_weights_sum_to_one():
+    """A closed curve subtends 2*pi at every interior point: sum_i (n.e/|e|^2) * (2*pi*R/S) -> 2*pi (trapezoid rule
+    on a periodic integrand: spectrally accurate).  Wrong exponent, sign or normal fails.  Centre: w = 1/S."""
+    n, h = (33, 33), 0.5e-3
+    origin = (-16 * h, -16 * h)
+    S, R = 256, 20e-3
+    sens, nrm = _ring(S, R)
+    w, om = oracle.solid_angle_weights(n, h, origin, sens, nrm, None, return_omega0=True)
+    np.testing.assert_allclose(om * (2 * np.pi * R / S), 2 * np.pi, rtol=1e-6)
+    np.testing.assert_allclose(w.astype(np.float64).sum(axis=0), 1.0, rtol=0, atol=2e-6)
+    centre = 16 * 33 + 16
+    np.testing.assert_allclose(w[:, centre], 1.0 / S, rtol=1e-6)
+    # off centre the nearer detectors weigh more (that is the whole point of the weighting)
+    j = 16 * 33 + 30                                                  # x = +7 mm
+    assert w[0, j] > 1.5 / S and w[S // 2, j] < 0.8 / S
+
+
+def test_p17_sphere_subtends_four_pi():
+    S, R = 4000, 20e-3
+    i = np.arange(S)
+    z = 1 - 2 * (i + 0.5) / S                                         # Fibonacci sphere: equal-area elements
+    ph = i * np.pi * (3 - np.sqrt(5))
+    rho = np.sqrt(1 - z * z)
+    nrm = np.stack([rho * np.cos(ph), rho * np.sin(ph), z], axis=1)
+    sens = (R * nrm).astype(np.float32)
+    n, h = (5, 5, 5), 2e-3
+    w, om = oracle.solid_angle_weights(n, h, (-2 * h,) * 3, sens, nrm.astype(np.float32), None, return_omega0=True)
+    np.testing.assert_allclose(om * (4 * np.pi * R * R / S), 4 * np.pi, rtol=2e-3)
+    np.testing.assert_allclose(w.astype(np.float64).sum(axis=0), 1.0, atol=1e-5)
+
+
+def test_p17_weights_brute_force_and_degenerate_cases():
+    rng = np.random.default_rng(21)
+    h = 2.0 ** -10                                                    # exactly representable coordinates
+    n, origin = (7, 6), (-3 * h, -2 * h)
+    S = 9
+    sens = np.zeros((S, 3), np.float32)
+    sens[:, :2] = rng.uniform(-8e-3, 8e-3, size=(S, 2))
+    nrm = np.zeros((S, 3), np.float32)
+    nrm[:, :2] = rng.standard_normal((S, 2))
+    sens[0, :2] = (origin[0] + 2 * h, origin[1] + 3 * h)              # a detector ON node (2, 3): weight 0 there
+    roi = np.sort(rng.choice(42, size=30, replace=False)).astype(np.int64)
+    roi[0] = 3 * 7 + 2
+    roi = np.unique(roi)
+    w = oracle.solid_angle_weights(n, h, origin, sens, nrm, roi)
+    ref = np.zeros((S, roi.size))
+    for jj, q in enumerate(roi):
+        r = np.array([np.float32(origin[0]) + np.float64(q % 7) * np.float32(h),
+                      np.float32(origin[1]) + np.float64(q // 7) * np.float32(h)], dtype=np.float64)
+        raw = np.zeros(S)
+        for i in range(S):
+            e = sens[i, :2].astype(np.float64) - r
+            dot = float(nrm[i, :2].astype(np.float64) @ e)
+            d2 = float(e @ e)
+            raw[i] = dot / d2 if (dot > 0 and d2 > 0) else 0.0
+        ref[:, jj] = raw / raw.sum() if raw.sum() > 0 else 0.0
+    np.testing.assert_allclose(w, ref, rtol=2e-7, atol=1e-12)
+    assert w[0, list(roi).index(3 * 7 + 2)] == 0.0
+    # all detectors facing away: all-zero weights, no NaN
+    w0 = oracle.solid_angle_weights(n, h, origin, np.array([[1.0, 0, 0]], np.float32), np.array([[-1.0, 0, 0]], np.float32), None)
+    assert np.all(w0 == 0.0)
+
+
+def test_p17_weighted_sum():
+    """w = 1: the plain sum; one-hot w: that sensor alone; linear in w; brute force."""
+    rng = np.random.default_rng(22)
+    tau, tr = _rand_case(rng, S=5, P=40, Nt=48, B=2, umax=49)
+    for mode in (0, 1, 2):
+        plain = oracle.backproject(tau, tr, FS, mode=mode)
+        np.testing.assert_allclose(oracle.backproject(tau, tr, FS, mode=mode, weights=np.ones_like(tau)), plain,
+                                   rtol=1e-13, atol=1e-13)
+    hot = np.zeros_like(tau)
+    hot[3] = 1.0
+    np.testing.assert_allclose(oracle.backproject(tau, tr, FS, weights=hot),
+                               oracle.backproject(tau[3:4], tr[:, 3:4], FS), rtol=1e-13, atol=1e-13)
+    w1 = rng.uniform(0, 1, tau.shape).astype(np.float32)
+    w2 = rng.uniform(0, 1, tau.shape).astype(np.float32)
+    w12 = (w1.astype(np.float64) + w2).astype(np.float32)
+    ok = w12.astype(np.float64) == w1.astype(np.float64) + w2                # keep the exactly representable sums
+    w1[~ok] = 0; w2[~ok] = 0; w12[~ok] = 0
+    np.testing.assert_allclose(oracle.backproject(tau, tr, FS, weights=w12),
+                               oracle.backproject(tau, tr, FS, weights=w1) + oracle.backproject(tau, tr, FS, weights=w2),
+                               rtol=1e-11, atol=1e-11)
+    # brute force: per-sensor images times the weights
+    acc = np.zeros((2, tau.shape[1]))
+    for i in range(tau.shape[0]):
+        acc += w1[i].astype(np.float64)[None, :] * _brute(tau[i:i + 1], tr[:, i:i + 1], FS, 1)
+    np.testing.assert_allclose(oracle.backproject(tau, tr, FS, weights=w1), acc, rtol=1e-11, atol=1e-11)
+
+
+def test_p17_large_ring_recovers_eq7():
+    """for a scanning radius much larger than the region, dOmega/Omega0 -> 1/S and the universal BP
+    becomes Eq. 7 / S."""
+    n, h = (9, 9), 0.25e-3
+    origin = (-4 * h, -4 * h)
+    S, R = 64, 1.0                                                     # 1 m ring around a 2 mm region
+    sens, nrm = _ring(S, R)
+    w = oracle.solid_angle_weights(n, h, origin, sens, nrm, None)
+    np.testing.assert_allclose(w * S, 1.0, rtol=3e-3)
+    rng = np.random.default_rng(23)
+    tau = (rng.uniform(2.0, 60.0, size=(S, 81)) / FS).astype(np.float32)
+    tr = rng.standard_normal((1, S, 64)).astype(np.float32)
+    a = oracle.backproject(tau, tr, FS, mode=2, weights=w) * S
+    b = oracle.backproject(tau, tr, FS, mode=2)
+    assert np.linalg.norm(a - b) <= 3e-3 * np.linalg.norm(b)
