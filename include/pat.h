@@ -147,6 +147,33 @@ pat_status pat_backproject_conventional(pat_plan *plan, const float *traces, flo
  * (rebuilt at the next call). */
 pat_status pat_set_roi_mask(pat_plan *plan, const uint8_t *mask);
 
+/* pat_set_pixel_weights -- SURVEY.md 8(f) NEXT-4: optional per-(sensor, pixel) factors w_ij that multiply every
+ * term of Eq. 7,  images[f][j] = sum_i w_ij * [(1-a)*b_fi[k] + a*b_fi[k+1]]  (Eq. 7 "can be viewed
+ * as an approximation to the exact BP algorithm [5]", whose terms carry the solid-angle factor
+ * dOmega_ij / Omega0_j; any other apodisation or directivity table goes the same way).
+ *   w   fp32 row-major [count][npix] (roi_index order) for sensors [sensor_begin, +count); HOST or DEVICE.
+ * The first call allocates a library-owned table of the size of the travel-time table (4*nsens*npix bytes,
+ * freed by pat_destroy), initialised to 1, and synchronises the device; rows not set stay 1.  From then on
+ * pat_backproject and pat_backproject_conventional stream the weight rows next to the delays.
+ * w = NULL with count = 0 removes the weights again (synchronises).
+ * Errors: bad range / NULL with count > 0 -> PAT_ERR_INVALID_ARG; a plan with an _EXACT weighting ->
+ * PAT_ERR_UNSUPPORTED; CUDA failure -> PAT_ERR_CUDA. */
+pat_status pat_set_pixel_weights(pat_plan *plan, const float *w, int32_t sensor_begin, int32_t count,
+                                 void *stream);
+
+/* pat_compute_solid_angle_weights -- fills the weight table with the universal BP's factors [5] computed on the
+ * device from the plan's geometry (fp64 from the fp32 inputs):
+ *     w_ij = dOmega_ij / sum_i' dOmega_i'j ,   dOmega_ij = n_i . (s_i - r_j) / |s_i - r_j|^3   (3-D)
+ *                                                          n_i . (s_i - r_j) / |s_i - r_j|^2   (2-D: subtended angle)
+ * with r_j = origin + index*h the ROI node, s_i the plan's sensor position and n_i the unit normal of the
+ * detection surface pointing away from the imaged region; a detector facing away (n.e <= 0) or sitting on the
+ * node gets 0, a node no detector faces gets all zeros (R27).  With weighting PAT_W_UBP this is the
+ * discretised universal back projection; for a ring much larger than the region w_ij -> 1/nsens.
+ *   normals  HOST fp32 [nsens*3], finite; read before the call returns (synchronises `stream`).
+ * Errors: NULL / non-finite normals -> PAT_ERR_INVALID_ARG; plan without sensor_xyz -> PAT_ERR_BAD_STATE;
+ * _EXACT weighting -> PAT_ERR_UNSUPPORTED. */
+pat_status pat_compute_solid_angle_weights(pat_plan *plan, const float *normals, void *stream);
+
 /* Frees the host-side plan; never frees caller memory.  NULL is allowed. */
 pat_status pat_destroy(pat_plan *plan);
 

@@ -84,6 +84,10 @@ def lib():
     L.pat_fmm_travel_times.argtypes = [gp, vp, vp, i32, vp, i64, i32, i32, i32, vp, i32]
     L.pat_compute_travel_times.restype = ctypes.c_int
     L.pat_compute_travel_times.argtypes = [vp, i32, i32, vp]
+    L.pat_set_pixel_weights.restype = ctypes.c_int
+    L.pat_set_pixel_weights.argtypes = [vp, vp, i32, i32, vp]
+    L.pat_compute_solid_angle_weights.restype = ctypes.c_int
+    L.pat_compute_solid_angle_weights.argtypes = [vp, vp, vp]
     L.pat_set_roi_mask.restype = ctypes.c_int
     L.pat_set_roi_mask.argtypes = [vp, vp]
     L.pat_backproject_conventional.restype = ctypes.c_int
@@ -160,6 +164,22 @@ def pat_backproject_conventional(plan, traces, images, nframes, c0, stream=None)
     """Eq. 7 with tau = |r - s| / c0 computed in the kernel."""
     return _check(plan, lib().pat_backproject_conventional(plan, _addr(traces), _addr(images), nframes,
                                                            float(c0), _stream(stream)))
+
+
+def pat_set_pixel_weights(plan, w, sensor_begin=0, count=None, stream=None):
+    """w: fp32 [count][npix] (numpy or torch) factors multiplying every term; None removes the weights."""
+    if w is None:
+        return _check(plan, lib().pat_set_pixel_weights(plan, None, 0, 0, _stream(stream)))
+    if isinstance(w, np.ndarray) and w.dtype != np.float32:
+        raise TypeError("w must be float32")
+    count = int(w.shape[0]) if count is None else count
+    return _check(plan, lib().pat_set_pixel_weights(plan, _addr(w), sensor_begin, count, _stream(stream)))
+
+
+def pat_compute_solid_angle_weights(plan, normals, stream=None):
+    """Universal-BP factors dOmega_ij/Omega0_j from the plan's geometry; normals: host fp32 [nsens][3]."""
+    normals = np.ascontiguousarray(normals, dtype=np.float32)
+    return _check(plan, lib().pat_compute_solid_angle_weights(plan, _addr(normals), _stream(stream)))
 
 
 def pat_set_roi_mask(plan, mask):
@@ -271,6 +291,12 @@ class Plan:
     def backproject_conventional(self, traces, images, c0, nframes=None, stream=None):
         nframes = int(traces.shape[0]) if nframes is None else nframes
         return pat_backproject_conventional(self.handle, traces, images, nframes, c0, stream)
+
+    def set_pixel_weights(self, w, sensor_begin=0, count=None, stream=None):
+        return pat_set_pixel_weights(self.handle, w, sensor_begin, count, stream)
+
+    def compute_solid_angle_weights(self, normals, stream=None):
+        return pat_compute_solid_angle_weights(self.handle, normals, stream)
 
     def set_roi_mask(self, mask):
         return pat_set_roi_mask(self.handle, mask)

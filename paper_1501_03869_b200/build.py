@@ -14,7 +14,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpat_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-         "-shared", "-Xcompiler", "-fPIC,-fopenmp,-O3,-Wall", "-cudart", "static"]
+         "-shared", "-Xcompiler", "-fPIC,-fopenmp,-O3,-Wall", "-cudart", "static", "--threads", "0"]
 
 
 def sources():

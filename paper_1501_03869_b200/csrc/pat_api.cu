@@ -269,7 +269,8 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
 pat_status get_schedule(pat_plan *p, int bp, bool onfly, PatSchedule **out) {
     for (PatSchedule &sc : p->schedules)
         if (sc.cfg.bp == bp && sc.cfg.onfly == onfly) { *out = &sc; return PAT_OK; }
-    PatGatherConfig cfg = pat_gather_config(bp, p->tune_wr, p->tune_R, p->tune_stages, onfly, p->exact);
+    PatGatherConfig cfg = pat_gather_config(bp, p->tune_wr, p->tune_R, p->tune_stages, onfly, p->exact,
+                                            p->d_w_t != nullptr);
     return build_schedule(p, cfg, out);
 }
 
@@ -482,6 +483,40 @@ extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, cons
     return PAT_OK;
 }
 
+// Rows [sensor_begin, +count) of a row-major [count][npix] table (host or device) -> the tile-major table
+// `dst_t`, every value mapped to fl32(fl32(v - t0) * fs) (fs = 1, t0 = 0: copied unchanged).
+static pat_status upload_rows(pat_plan *p, const float *src, int32_t sensor_begin, int32_t count, float *dst_t,
+                              float fs, float t0, void *stream) {
+    const int on_dev = is_device_ptr(src);
+    if (on_dev < 0) return fail(p, PAT_ERR_CUDA, "cudaPointerGetAttributes failed on the table rows");
+    cudaStream_t st = (cudaStream_t)stream;
+    PatLaunchCtx ctx{stream, p->num_sms, p->use_pdl};
+    const int32_t *perm = (const int32_t *)(p->ws + p->lay.perm);
+    const int64_t P = p->dims.npix;
+    if (on_dev) {
+        int e = pat_launch_retile(ctx, src, dst_t, perm, p->dims.nsens, P, p->dims.ntiles, sensor_begin, count, fs, t0);
+        if (e) return cuda_fail(p, e, "retile launch");
+        ++p->launches;
+    } else {
+        float *stage = (float *)(p->ws + p->lay.tau_stage);
+        for (int32_t r = 0; r < count; r += (int32_t)p->lay.stage_rows) {
+            const int32_t m = (int32_t)std::min<int64_t>(p->lay.stage_rows, count - r);
+            cudaError_t e = cudaMemcpyAsync(stage, src + (int64_t)r * P, (size_t)m * P * sizeof(float),
+                                            cudaMemcpyHostToDevice, st);
+            if (e != cudaSuccess) return cuda_fail(p, e, "table H2D copy");
+            int le = pat_launch_retile(ctx, stage, dst_t, perm, p->dims.nsens, P, p->dims.ntiles,
+                                       sensor_begin + r, m, fs, t0);
+            if (le) return cuda_fail(p, le, "retile launch");
+            ++p->launches;
+            // the staging buffer is reused by the next piece and the host rows are only
+            // borrowed until return: wait for this piece.
+            e = cudaStreamSynchronize(st);
+            if (e != cudaSuccess) return cuda_fail(p, e, "table staging synchronise");
+        }
+    }
+    return PAT_OK;
+}
+
 extern "C" pat_status pat_set_travel_times(pat_plan *p, const float *tau, int32_t sensor_begin,
                                            int32_t count, void *stream) {
     if (!p) return PAT_ERR_INVALID_ARG;
@@ -489,35 +524,8 @@ extern "C" pat_status pat_set_travel_times(pat_plan *p, const float *tau, int32_
     if (sensor_begin < 0 || count < 0 || sensor_begin > p->dims.nsens - count)
         return fail(p, PAT_ERR_INVALID_ARG, "sensor range outside [0, nsens)");
     if (count == 0) return PAT_OK;
-    const int on_dev = is_device_ptr(tau);
-    if (on_dev < 0) return fail(p, PAT_ERR_CUDA, "cudaPointerGetAttributes failed on tau");
-    cudaStream_t st = (cudaStream_t)stream;
-    PatLaunchCtx ctx{stream, p->num_sms, p->use_pdl};
-    float *tau_t = (float *)(p->ws + p->lay.tau);
-    const int32_t *perm = (const int32_t *)(p->ws + p->lay.perm);
-    const int64_t P = p->dims.npix;
-    if (on_dev) {
-        int e = pat_launch_retile(ctx, tau, tau_t, perm, p->dims.nsens, P, p->dims.ntiles, sensor_begin, count,
-                                  p->fs, p->t0);
-        if (e) return cuda_fail(p, e, "retile launch");
-        ++p->launches;
-    } else {
-        float *stage = (float *)(p->ws + p->lay.tau_stage);
-        for (int32_t r = 0; r < count; r += (int32_t)p->lay.stage_rows) {
-            const int32_t m = (int32_t)std::min<int64_t>(p->lay.stage_rows, count - r);
-            cudaError_t e = cudaMemcpyAsync(stage, tau + (int64_t)r * P, (size_t)m * P * sizeof(float),
-                                            cudaMemcpyHostToDevice, st);
-            if (e != cudaSuccess) return cuda_fail(p, e, "tau H2D copy");
-            int le = pat_launch_retile(ctx, stage, tau_t, perm, p->dims.nsens, P, p->dims.ntiles,
-                                       sensor_begin + r, m, p->fs, p->t0);
-            if (le) return cuda_fail(p, le, "retile launch");
-            ++p->launches;
-            // the staging buffer is reused by the next piece and the host rows are only
-            // borrowed until return: wait for this piece.
-            e = cudaStreamSynchronize(st);
-            if (e != cudaSuccess) return cuda_fail(p, e, "tau staging synchronise");
-        }
-    }
+    pat_status us = upload_rows(p, tau, sensor_begin, count, (float *)(p->ws + p->lay.tau), p->fs, p->t0, stream);
+    if (us != PAT_OK) return us;
     for (int32_t s = sensor_begin; s < sensor_begin + count; ++s)
         if (!p->row_set[s]) { p->row_set[s] = 1; ++p->rows_set; }
     p->meta_valid = false;
@@ -638,7 +646,7 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
                               sc->grid_x, p->d_perm_masked ? p->d_perm_masked : (const int32_t *)(p->ws + p->lay.perm),
                               d_img, d.nsens, d.npix, d.nt,
                               p->nt4, nframes, p->trace_ctas == sc->grid_x ? p->trace_dev : nullptr,
-                              conventional ? &onfly : nullptr, t0fs);
+                              conventional ? &onfly : nullptr, t0fs, p->d_w_t);
         if (e) return cuda_fail(p, e, "gather launch");
         ++p->launches;
     }
@@ -668,6 +676,7 @@ extern "C" pat_status pat_destroy(pat_plan *p) {
     if (p) {
         drop_events(p); drop_schedules(p);
         if (p->d_perm_masked) cudaFree(p->d_perm_masked);
+        if (p->d_w_t) cudaFree(p->d_w_t);
         if (p->d_pix) cudaFree(p->d_pix);
         if (p->d_sens) cudaFree(p->d_sens);
         if (p->copy_stream) { cudaStreamSynchronize((cudaStream_t)p->copy_stream); cudaStreamDestroy((cudaStream_t)p->copy_stream); }
@@ -765,6 +774,89 @@ extern "C" pat_status pat_compute_travel_times_gpu(pat_plan *p, int32_t max_roun
         if (cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) return fail(p, PAT_ERR_CUDA, "synchronise");
     }
     if (rounds_out) *rounds_out = worst;
+    return PAT_OK;
+}
+
+// The weight table exists from the first call on (all ones = no effect) and is library-owned.
+static pat_status ensure_weight_table(pat_plan *p, void *stream) {
+    if (p->exact)
+        return fail(p, PAT_ERR_UNSUPPORTED, "pixel weights are not available with the _EXACT weightings");
+    if (p->d_w_t) return PAT_OK;
+    cudaError_t e = cudaDeviceSynchronize();            // no launch may still use the unweighted work lists
+    if (e != cudaSuccess) return cuda_fail(p, e, "synchronise");
+    const int64_t n = p->dims.ntiles * (int64_t)p->dims.nsens * kTilePix;
+    e = cudaMalloc((void **)&p->d_w_t, (size_t)n * sizeof(float));
+    if (e != cudaSuccess) { p->d_w_t = nullptr; return cuda_fail(p, e, "weight table allocation"); }
+    PatLaunchCtx ctx{stream, p->num_sms, false};
+    int le = pat_launch_fill(ctx, p->d_w_t, n, 1.0f);
+    if (le) { cudaFree(p->d_w_t); p->d_w_t = nullptr; return cuda_fail(p, le, "weight table fill"); }
+    ++p->launches;
+    drop_schedules(p);                                  // the stages now hold weight rows as well
+    return PAT_OK;
+}
+
+extern "C" pat_status pat_set_pixel_weights(pat_plan *p, const float *w, int32_t sensor_begin, int32_t count,
+                                            void *stream) {
+    if (!p) return PAT_ERR_INVALID_ARG;
+    if (!w) {                                           // remove the weights
+        if (count != 0) return fail(p, PAT_ERR_INVALID_ARG, "w is NULL");
+        if (p->d_w_t) {
+            cudaError_t e = cudaDeviceSynchronize();
+            if (e != cudaSuccess) return cuda_fail(p, e, "synchronise");
+            cudaFree(p->d_w_t);
+            p->d_w_t = nullptr;
+            drop_schedules(p);
+        }
+        return PAT_OK;
+    }
+    if (sensor_begin < 0 || count < 0 || sensor_begin > p->dims.nsens - count)
+        return fail(p, PAT_ERR_INVALID_ARG, "sensor range outside [0, nsens)");
+    pat_status st = ensure_weight_table(p, stream);
+    if (st != PAT_OK || count == 0) return st;
+    return upload_rows(p, w, sensor_begin, count, p->d_w_t, 1.0f, 0.0f, stream);
+}
+
+extern "C" pat_status pat_compute_solid_angle_weights(pat_plan *p, const float *normals, void *stream) {
+    if (!p) return PAT_ERR_INVALID_ARG;
+    if (!normals) return fail(p, PAT_ERR_INVALID_ARG, "normals is NULL");
+    if (p->sensors.empty()) return fail(p, PAT_ERR_BAD_STATE, "plan was created without sensor_xyz");
+    const int32_t S = p->dims.nsens;
+    for (int64_t q = 0; q < (int64_t)S * 3; ++q)
+        if (!std::isfinite(normals[q])) return fail(p, PAT_ERR_INVALID_ARG, "normals must be finite");
+    pat_status st = ensure_weight_table(p, stream);
+    if (st != PAT_OK) return st;
+    // node coordinates of every tile slot in double: x_d = origin_d + i_d * h from the fp32 grid data
+    const int64_t slots = p->dims.ntiles * kTilePix;
+    std::vector<double> pix;
+    try { pix.assign((size_t)slots * 3, 0.0); } catch (...) { return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
+    const int64_t n0 = p->grid.n[0], n1 = p->grid.n[1];
+    for (int64_t sl = 0; sl < slots; ++sl) {
+        int32_t pos = p->host_perm[(size_t)sl];
+        if (pos < 0) pos = p->host_perm[(size_t)(sl / kTilePix * kTilePix)];          // padding: the tile's first pixel
+        const int64_t q = p->roi.empty() ? pos : p->roi[(size_t)pos];
+        const int64_t id[3] = {q % n0, (q / n0) % n1, q / (n0 * n1)};
+        for (int dd = 0; dd < p->grid.ndim; ++dd)
+            pix[(size_t)dd * slots + sl] = (double)p->grid.origin[dd] + (double)id[dd] * (double)p->grid.h;
+    }
+    double *d_pix = nullptr;
+    float *d_sn = nullptr;                              // sensors, then normals
+    cudaStream_t cs = (cudaStream_t)stream;
+    cudaError_t e = cudaMalloc((void **)&d_pix, pix.size() * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&d_sn, (size_t)S * 6 * sizeof(float));
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_pix, pix.data(), pix.size() * sizeof(double), cudaMemcpyHostToDevice, cs);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_sn, p->sensors.data(), (size_t)S * 3 * sizeof(float), cudaMemcpyHostToDevice, cs);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_sn + (size_t)S * 3, normals, (size_t)S * 3 * sizeof(float), cudaMemcpyHostToDevice, cs);
+    int le = 0;
+    if (e == cudaSuccess) {
+        PatLaunchCtx ctx{stream, p->num_sms, false};
+        le = pat_launch_solid_angle(ctx, d_pix, slots, d_sn, d_sn + (size_t)S * 3, S, p->grid.ndim, p->d_w_t);
+        ++p->launches;
+    }
+    if (e == cudaSuccess && !le) e = cudaStreamSynchronize(cs);       // the host arrays are only borrowed
+    cudaFree(d_pix);
+    cudaFree(d_sn);
+    if (le) return cuda_fail(p, le, "solid-angle launch");
+    if (e != cudaSuccess) return cuda_fail(p, e, "solid-angle weights");
     return PAT_OK;
 }
 

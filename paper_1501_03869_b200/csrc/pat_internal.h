@@ -49,6 +49,7 @@ struct PatGatherConfig {
     uint32_t hdr_bytes = 0, stage_bytes = 0;
     bool onfly = false;       // work list of the conventional BP (k-ranges from the geometry, no table)
     bool exact = false;       // PAT_W_*_EXACT: the bp "frames" are channel pairs {wp*p, -wd*D} of bp/2 frames
+    bool weighted = false;    // pat_set_pixel_weights: a stage holds R weight rows after its R u rows
 };
 
 // Conventional BP: tau = |r - s| / c0 computed inside the gather.
@@ -104,6 +105,8 @@ struct pat_plan {
     float *d_pix = nullptr, *d_sens = nullptr;
     float onfly_c0 = 0;
     std::vector<int32_t> onfly_meta;
+    // pat_set_pixel_weights / pat_compute_solid_angle_weights: per-(sensor, pixel) factors, tile-major like u_t
+    float *d_w_t = nullptr;           // library-owned [ntiles][nsens][256], NULL = no weights
     // pat_set_roi_mask: tiles without a selected pixel leave the work lists; unselected pixels are not written
     std::vector<uint8_t> tile_active;   // empty = everything
     int32_t *d_perm_masked = nullptr;   // [ntiles*256] perm with the unselected pixels set to -1
@@ -144,7 +147,8 @@ int pat_launch_stream_probe(const PatLaunchCtx &ctx, const void *a, int64_t a_by
 int pat_frames_per_group(int32_t nframes);
 bool pat_gather_blocked(int bp);       // trace layout [sensor][n/32][frame][32] instead of [sensor][n][frame]
 int pat_gather_wrmax(int bp);          // default / largest slot window for this frame-count class
-PatGatherConfig pat_gather_config(int bp, int wr, int R, int stages, bool onfly = false, bool exact = false);   // 0 = choose automatically
+PatGatherConfig pat_gather_config(int bp, int wr, int R, int stages, bool onfly = false, bool exact = false,
+                                  bool weighted = false);   // 0 = choose automatically
 size_t pat_gather_smem_bytes(const PatGatherConfig &c);
 int pat_gather_occupancy(const PatGatherConfig &c, int *per_sm);
 int pat_launch_gather(const PatLaunchCtx &ctx, const PatGatherConfig &c, const float *u_t, const float *b,
@@ -152,7 +156,15 @@ int pat_launch_gather(const PatLaunchCtx &ctx, const PatGatherConfig &c, const f
                       float *images, int32_t nsens, int64_t npix, int32_t nt, int32_t nt4, int32_t nframes,
                       unsigned long long *trace = nullptr,    // trace: per-CTA timeline, 8 x u64 per CTA, or NULL
                       const PatOnfly *onfly = nullptr,        // conventional BP: u computed in the kernel
-                      float t0fs = 0.0f);                     // exact-time weightings: t0*fs
+                      float t0fs = 0.0f,                      // exact-time weightings: t0*fs
+                      const float *w_t = nullptr);            // pixel weights [ntiles][nsens][256] (cfg.weighted)
+
+// Set-up kernels of the pixel weights (weights.cu).
+int pat_launch_fill(const PatLaunchCtx &ctx, float *dst, int64_t n, float value);
+// Universal-BP solid-angle weights dOmega_ij / Omega0_j straight into the tile-major table: pix = double
+// [3][slots] node coordinates per tile slot, sens / nrm = float [nsens][3] (all device).
+int pat_launch_solid_angle(const PatLaunchCtx &ctx, const double *pix, int64_t slots, const float *sens,
+                           const float *nrm, int32_t nsens, int32_t ndim, float *w_t);
 int pat_launch_onfly_meta(const PatLaunchCtx &ctx, const PatOnfly &o, int32_t nsens, void *meta, int64_t nrows, int32_t nt);
 
 #endif  // PAT_INTERNAL_H_
