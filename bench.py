@@ -20,6 +20,7 @@ CPU FMM (input preparation, untimed).  Prints ONE JSON line (rank 0):
   large_workload_probe  the same path on configs[4] reduced (537 MB table): the gather's steady-state rate.
   conventional_bp  PAPER.md:69's comparison method with the delays computed in the kernel (no table stream).
   exact_time_weighting  Eq. 7 with p and dp/dt both taken at t_ij (PAT_W_PAPER_EXACT, two channels per frame).
+  universal_bp     ref. [5]'s solid-angle-weighted sum: a weight table streamed next to the delays.
   offline_eikonal  (not part of the step) the tau table of the geometry solved on the GPU vs the CPU fast marching.
   sweep        B = 1..64 on the same geometry (N = 1 only): ms/frame, GUpd/s, HBM fraction and the
                SM-side (shared-memory bandwidth) fraction, because for B >~ 4 the path is not
@@ -62,7 +63,7 @@ def parse_args():
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--probe", default="", choices=["", "conventional", "eikonal", "exact"],
+    ap.add_argument("--probe", default="", choices=["", "conventional", "eikonal", "exact", "ubp"],
                     help="run only this side probe on the config's geometry and print its JSON (ncu captures)")
     ap.add_argument("--tuning", type=str, default="", help="wr,rows,stages for pat_set_gather_tuning (0 = automatic)")
     return ap.parse_args()
@@ -243,11 +244,34 @@ def exact_time_probe(geom, tau, traces, peak_gbs, batches=(1, 16), steps=400):
     return out
 
 
+def universal_bp_probe(geom, tau, traces, peak_gbs, batches=(1, 32), steps=400):
+    """the universal BP of ref. [5] = weighting 2p - 2t dp/dt with every term
+    multiplied by dOmega_ij/Omega0_j (pat_compute_solid_angle_weights, radial normals): a second table of the size
+    of the delays is streamed, so the algorithmic bytes are tau + weights + traces + images."""
+    import paper_1501_03869_b200 as pat
+    s = geom.sensors.astype(np.float64)
+    nrm = (s / np.linalg.norm(s, axis=1, keepdims=True)).astype(np.float32)
+    out = []
+    for B in batches:
+        rig = Rig(geom, tau, traces, B, weighting=pat.PAT_W_UBP, normals=nrm)
+        rig.run(rig.R)
+        rig.torch.cuda.synchronize()
+        rig.capture_round()
+        n = max(20, steps // B)
+        ms = time_steps(rig, n, 10) / n
+        rig.close()
+        upd = float(B) * geom.nsens * geom.npix
+        nbytes = algorithmic_bytes(geom.nsens, geom.npix, geom.nt, B) + 4.0 * geom.nsens * geom.npix
+        out.append({"B": B, "ms_per_frame": round(ms / B, 6), "gupd_s": round(upd / (ms * 1e-3) / 1e9, 1),
+                    "step_hbm_frac": round(nbytes / (ms * 1e-3) / 1e9 / peak_gbs, 4)})
+    return out
+
+
 class Rig:
     """R rotating plans (own tau copy, traces, images) so that consecutive steps never find their
     tau table in L2: R * tau bytes > 3 x L2."""
 
-    def __init__(self, geom, tau, traces, B, variant=0, host=False, weighting=None):
+    def __init__(self, geom, tau, traces, B, variant=0, host=False, weighting=None, normals=None):
         import torch
         import paper_1501_03869_b200 as pat
         self.pat, self.torch, self.geom, self.B = pat, torch, geom, B
@@ -267,6 +291,8 @@ class Rig:
             if variant:
                 pat.pat_set_gather_tuning(p.handle, *variant)
             p.set_travel_times(tau)
+            if normals is not None:                            # universal BP: solid-angle table next to the delays
+                p.compute_solid_angle_weights(normals)
             sel = [(r * B + f) % F for f in range(B)]
             t = torch.from_numpy(np.ascontiguousarray(traces[sel]))
             if host:
@@ -494,6 +520,9 @@ def run_ours(args):
     if args.probe:                                       # SURVEY.md 8(f) rows, off the headline path
         if args.probe == "eikonal":
             print(json.dumps({"offline_eikonal": eikonal_probe(geom0)}))
+        elif args.probe == "ubp":
+            g1, tau1, tr1 = prepare_inputs(k, args.reduced, max(1, args.batch or 1))
+            print(json.dumps({"universal_bp": universal_bp_probe(g1, tau1, tr1, peak_gbs, batches=(args.batch or 1,))}))
         elif args.probe == "exact":
             g1, tau1, tr1 = prepare_inputs(k, args.reduced, max(1, args.batch or 1))
             print(json.dumps({"exact_time_weighting": exact_time_probe(g1, tau1, tr1, peak_gbs, batches=(args.batch or 1,))}))
@@ -538,11 +567,12 @@ def run_ours(args):
                  "ms_per_frame": round(m4["ms_per_frame"], 6), "gupd_s": round(m4["gupd_s"], 1),
                  "step_hbm_frac": round(m4["step_hbm_frac"], 4), "gather_hbm_frac": round(m4["gather_gbs"] / peak_gbs, 4),
                  "full_size_result": "profiles/r01_config4_full.md (34.4 GB table: 6.26 ms/frame, 0.84 of the HBM peak)"}
-    eik, conv, exact = None, None, None
+    eik, conv, exact, ubp = None, None, None, None
     if do_sweep:
         eik = eikonal_probe(geom)
         conv = conventional_probe(geom, traces)
         exact = exact_time_probe(geom, tau, traces, peak_gbs)
+        ubp = universal_bp_probe(geom, tau, traces, peak_gbs)
     sampler.stop_flag = True
     sampler.join(timeout=2.0)
     clocks_main = sampler.summary()
@@ -595,6 +625,8 @@ def run_ours(args):
         line["conventional_bp"] = conv
     if exact:
         line["exact_time_weighting"] = exact
+    if ubp:
+        line["universal_bp"] = ubp
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(geom, tau, traces)
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
