@@ -419,7 +419,8 @@ def measure(geom, tau, traces, B, steps, warmup, variant, dist, peak_gbs, sm_mhz
         ms_h = time_steps(hrig, n_e2e, min(warmup, 10), dist)
         out["e2e_gupd_s"] = upd * n_e2e / (ms_h * 1e-3) / 1e9
         out["e2e_ms_per_step"] = ms_h / n_e2e
-        out["h2d"] = 4 * B * S * Nt
+        out["trace_window"] = list(hrig.plans[0].trace_window())      # samples of every trace that cross the bus
+        out["h2d"] = 4 * B * S * out["trace_window"][1]
         out["d2h"] = 4 * B * P
         hrig.close()
     return out
@@ -614,6 +615,8 @@ def run_ours(args):
     if "e2e_gupd_s" in main:
         line["e2e"] = {"value": main["e2e_gupd_s"] * world, "unit": "GUpd/s",
                        "h2d_bytes_per_step": main["h2d"], "d2h_bytes_per_step": main["d2h"],
+                       "trace_samples_transferred": "[%d, +%d) of %d: all the table can touch (pat_get_trace_window)"
+                                                    % (main["trace_window"][0], main["trace_window"][1], Nt),
                        "ms_per_step": main["e2e_ms_per_step"]}
     if sweep:
         line["sweep"] = sweep

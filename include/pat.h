@@ -118,7 +118,8 @@ pat_status pat_set_travel_times(pat_plan *plan, const float *tau, int32_t sensor
  * copy stream owned by the plan into one of two staging buffers and `stream` waits for that copy, so
  * the transfer of one call runs under the kernels of the previous call; everything is complete when
  * `stream` is (the host traces must stay untouched until then).  Inside a stream capture, or with
- * PAT_NO_PIPE=1, the copy is simply enqueued on `stream`.
+ * PAT_NO_PIPE=1, the copy is simply enqueued on `stream`.  Only the samples the table can touch are
+ * transferred (pat_get_trace_window).
  * With PAT_W_PAPER_EXACT / PAT_W_UBP_EXACT the term is the one stated at pat_weighting (two channels per
  * frame through the same kernels) and nframes <= max_batch/2.
  * nframes = 0 is a no-op; nframes > max_batch (> max_batch/2 for the _EXACT weightings) ->
@@ -182,6 +183,14 @@ pat_status pat_destroy(pat_plan *plan);
 /* Last error text of a plan (or of the last failed pat_plan_create when plan == NULL).
  * Never NULL; owned by the library. */
 const char *pat_last_error(const pat_plan *plan);
+
+/* The part of every trace the uploaded table can touch: samples [first, first+count) hold b[k], b[k+1] of every valid
+ * (sensor, pixel) pair plus the +-1 halo of the central difference (rounded to whole 16-byte quads).  A
+ * pat_backproject call with HOST buffers transfers only this part of every trace (one strided copy) when it is at
+ * most 80 % of the record -- the paper's frame times include the transfers, and on configs[1] a pixel
+ * inside the skull can only be reached by about a quarter of the 2048 samples; otherwise, or with
+ * PAT_FULL_H2D=1, first = 0 and count = nt.  PAT_ERR_BAD_STATE until every tau row has been set. */
+pat_status pat_get_trace_window(const pat_plan *plan, int32_t *first, int32_t *count);
 
 /* Number of kernels of this library launched through `plan` so far (monotone counter). */
 int64_t pat_kernel_launches(const pat_plan *plan);

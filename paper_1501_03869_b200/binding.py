@@ -84,6 +84,8 @@ def lib():
     L.pat_fmm_travel_times.argtypes = [gp, vp, vp, i32, vp, i64, i32, i32, i32, vp, i32]
     L.pat_compute_travel_times.restype = ctypes.c_int
     L.pat_compute_travel_times.argtypes = [vp, i32, i32, vp]
+    L.pat_get_trace_window.restype = ctypes.c_int
+    L.pat_get_trace_window.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i32)]
     L.pat_set_pixel_weights.restype = ctypes.c_int
     L.pat_set_pixel_weights.argtypes = [vp, vp, i32, i32, vp]
     L.pat_compute_solid_angle_weights.restype = ctypes.c_int
@@ -164,6 +166,13 @@ def pat_backproject_conventional(plan, traces, images, nframes, c0, stream=None)
     """Eq. 7 with tau = |r - s| / c0 computed in the kernel."""
     return _check(plan, lib().pat_backproject_conventional(plan, _addr(traces), _addr(images), nframes,
                                                            float(c0), _stream(stream)))
+
+
+def pat_get_trace_window(plan):
+    """(first, count): the samples of every trace a host-buffer call transfers (all the table can touch)."""
+    a, b = ctypes.c_int32(), ctypes.c_int32()
+    _check(plan, lib().pat_get_trace_window(plan, ctypes.byref(a), ctypes.byref(b)))
+    return a.value, b.value
 
 
 def pat_set_pixel_weights(plan, w, sensor_begin=0, count=None, stream=None):
@@ -297,6 +306,9 @@ class Plan:
 
     def compute_solid_angle_weights(self, normals, stream=None):
         return pat_compute_solid_angle_weights(self.handle, normals, stream)
+
+    def trace_window(self):
+        return pat_get_trace_window(self.handle)
 
     def set_roi_mask(self, mask):
         return pat_set_roi_mask(self.handle, mask)

@@ -70,6 +70,21 @@ inline uint64_t spread3(uint32_t v) {
     return x;
 }
 
+// Samples [lo, hi) of a trace that the rows of `meta` ({kmin, kmax | flags} per row) can touch: b[kmin .. kmax+1],
+// i.e. p[kmin-1 .. kmax+2] with the central difference, rounded outwards to whole 16-byte quads.
+void needed_samples(const std::vector<int32_t> &meta, int32_t nt, int32_t *lo, int32_t *hi) {
+    int32_t kmin = INT32_MAX, kmax = -1;
+    for (size_t r = 0; r + 1 < meta.size(); r += 2) {
+        const int32_t a = meta[r], b = meta[r + 1] < 0 ? -1 : (meta[r + 1] & 0x3FFFFFFF);
+        if (b < a) continue;
+        kmin = std::min(kmin, a);
+        kmax = std::max(kmax, b);
+    }
+    if (kmax < 0) { *lo = *hi = 0; return; }                // no valid entry at all: nothing is read
+    *lo = std::max(0, kmin - 1) & ~3;
+    *hi = std::min(nt, (kmax + 3 + 3) & ~3);
+}
+
 void drop_schedules(pat_plan *p) {
     for (PatSchedule &sc : p->schedules) {
         if (sc.d_sched) cudaFree(sc.d_sched);
@@ -92,6 +107,7 @@ pat_status finalize_table(pat_plan *p, void *stream) {
     if (ce == cudaSuccess) ce = cudaStreamSynchronize((cudaStream_t)stream);
     if (ce != cudaSuccess) return cuda_fail(p, ce, "row-meta read-back");
     p->meta_valid = true;
+    needed_samples(p->host_meta, p->dims.nt, &p->need_lo, &p->need_hi);
     return PAT_OK;
 }
 
@@ -321,6 +337,7 @@ pat_status ensure_onfly(pat_plan *p, float c0, void *stream, PatOnfly *out) {
         cudaFree(d_meta);
         if (le || e != cudaSuccess) { p->onfly_meta.clear(); return cuda_fail(p, le ? le : (int)e, "conventional BP row ranges"); }
         p->onfly_c0 = c0;
+        needed_samples(p->onfly_meta, p->dims.nt, &p->onfly_lo, &p->onfly_hi);
         // work lists of the previous c0 are stale
         for (size_t q = 0; q < p->schedules.size();) {
             if (p->schedules[q].cfg.onfly) {
@@ -421,6 +438,8 @@ extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, cons
     p->ws = (char *)workspace;
     const char *env = std::getenv("PAT_NO_PDL");
     p->use_pdl = !(env && env[0] == '1');
+    env = std::getenv("PAT_FULL_H2D");                     // A/B switch: always transfer whole traces
+    p->window_h2d = !(env && env[0] == '1');
 
     std::vector<int32_t> perm;
     try {
@@ -574,10 +593,27 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
     float *d_img = images;
     const int slot = (int)(p->host_calls & 1u);
     bool piped = false;
+    PatOnfly onfly;
+    if (conventional) {      // geometry + k-ranges for this c0 (first use: builds them, synchronous)
+        pat_status os = ensure_onfly(p, c0, stream, &onfly);
+        if (os != PAT_OK) return os;
+    }
     if (!td) {
         d_tr = (const float *)(p->ws + (slot ? p->lay.traces2 : p->lay.traces));
         d_img = (float *)(p->ws + p->lay.images);
         const size_t tbytes = (size_t)nframes * d.nsens * d.nt * sizeof(float);
+        // only the samples the table can touch cross the bus (PAPER.md:79 counts the transfers): one strided copy
+        // of [lo, hi) of every trace when that is well below the whole record; the rest of the staging buffer is
+        // never read by a valid pixel
+        const int32_t lo = conventional ? p->onfly_lo : p->need_lo, hi = conventional ? p->onfly_hi : p->need_hi;
+        const bool windowed = p->window_h2d && (int64_t)(hi - lo) * 5 <= (int64_t)d.nt * 4;
+        auto h2d = [&](cudaStream_t s_) -> cudaError_t {
+            if (!windowed) return cudaMemcpyAsync((void *)d_tr, traces, tbytes, cudaMemcpyHostToDevice, s_);
+            if (hi <= lo) return cudaSuccess;
+            return cudaMemcpy2DAsync((void *)(d_tr + lo), (size_t)d.nt * sizeof(float), traces + lo,
+                                     (size_t)d.nt * sizeof(float), (size_t)(hi - lo) * sizeof(float),
+                                     (size_t)nframes * d.nsens, cudaMemcpyHostToDevice, s_);
+        };
         cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
         cudaStreamIsCapturing(st, &cap);
         piped = p->copy_stream && cap == cudaStreamCaptureStatusNone;
@@ -587,23 +623,18 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
             // overwrite this staging buffer once the pre-pass of the call before last has read it
             cudaStream_t cs = (cudaStream_t)p->copy_stream;
             e = p->host_calls >= 2 ? cudaStreamWaitEvent(cs, (cudaEvent_t)p->ev_read[slot], 0) : cudaSuccess;
-            if (e == cudaSuccess) e = cudaMemcpyAsync((void *)d_tr, traces, tbytes, cudaMemcpyHostToDevice, cs);
+            if (e == cudaSuccess) e = h2d(cs);
             if (e == cudaSuccess) e = cudaEventRecord((cudaEvent_t)p->ev_h2d[slot], cs);
             if (e == cudaSuccess) e = cudaStreamWaitEvent(st, (cudaEvent_t)p->ev_h2d[slot], 0);
         } else {
-            e = cudaMemcpyAsync((void *)d_tr, traces, tbytes, cudaMemcpyHostToDevice, st);
+            e = h2d(st);
         }
         if (e != cudaSuccess) return cuda_fail(p, e, "traces H2D copy");
         ++p->host_calls;
     }
     const int bp = pat_frames_per_group(nch);
     PatSchedule *sc = nullptr;
-    PatOnfly onfly;
     {   // first use of this frame-count class after the table (or c0) changed: builds the work list (synchronous)
-        if (conventional) {
-            pat_status os = ensure_onfly(p, c0, stream, &onfly);
-            if (os != PAT_OK) return os;
-        }
         pat_status ss = get_schedule(p, bp, conventional, &sc);
         if (ss != PAT_OK) return ss;
     }
@@ -722,6 +753,16 @@ extern "C" const char *pat_last_error(const pat_plan *p) {
 }
 
 extern "C" int64_t pat_kernel_launches(const pat_plan *p) { return p ? p->launches : 0; }
+
+extern "C" pat_status pat_get_trace_window(const pat_plan *p, int32_t *first, int32_t *count) {
+    if (!p || !first || !count) return PAT_ERR_INVALID_ARG;
+    if (!p->meta_valid) return PAT_ERR_BAD_STATE;
+    const int32_t lo = p->need_lo, hi = p->need_hi;
+    const bool windowed = p->window_h2d && (int64_t)(hi - lo) * 5 <= (int64_t)p->dims.nt * 4;
+    *first = windowed ? lo : 0;
+    *count = windowed ? hi - lo : p->dims.nt;
+    return PAT_OK;
+}
 
 extern "C" pat_status pat_set_gather_tuning(pat_plan *p, int32_t wr, int32_t rows, int32_t stages) {
     if (!p) return PAT_ERR_INVALID_ARG;

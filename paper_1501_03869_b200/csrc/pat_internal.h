@@ -84,6 +84,7 @@ struct pat_plan {
     int num_sms = 0;
     int tune_wr = 0, tune_R = 0, tune_stages = 0;   // pat_set_gather_tuning overrides (0 = automatic)
     bool use_pdl = true;
+    bool window_h2d = true;           // host traces: copy only the samples the table can touch (PAT_FULL_H2D=1: all)
     std::vector<uint8_t> row_set;     // per sensor: tau row uploaded?
     int64_t rows_set = 0;
     bool meta_valid = false;          // host_meta matches the uploaded table
@@ -100,6 +101,10 @@ struct pat_plan {
     void *copy_stream = nullptr;
     void *ev_h2d[2] = {nullptr, nullptr}, *ev_read[2] = {nullptr, nullptr};
     uint64_t host_calls = 0;
+    // samples [need_lo, need_hi) of a trace are all the table can touch (k-ranges of every row plus the
+    // derivative's +-1 halo, rounded to 4 samples): host-buffer calls transfer only that part of every trace
+    int32_t need_lo = 0, need_hi = 0;        // table path; valid when meta_valid
+    int32_t onfly_lo = 0, onfly_hi = 0;      // conventional BP, for onfly_c0
     // conventional BP (pat_backproject_conventional): geometry on the device, k-ranges for the current c0
     std::vector<int32_t> host_perm;   // tile slot -> ROI position (-1 = padding)
     float *d_pix = nullptr, *d_sens = nullptr;

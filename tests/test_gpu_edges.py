@@ -280,3 +280,42 @@ def test_roi_mask_selects_pixels_without_touching_the_table():
             assert_parity(img.cpu().numpy(), ref, "mask removed")
         finally:
             plan.close()
+
+
+@pytest.mark.parametrize("lo_u,hi_u,expect", [(300.0, 700.0, (296, 408)), (0.0, 2046.0, (0, 2048)), (5.0, 9.0, (4, 8))])
+def test_host_calls_transfer_only_the_samples_the_table_can_touch(lo_u, hi_u, expect):
+    """pat_get_trace_window / PAPER.md:79 (the frame time includes the transfers): with host buffers only the
+    samples [kmin-1, kmax+2] (rounded to quads) of every trace cross the bus.  The workspace is poisoned with NaN
+    bit patterns beforehand, so anything read outside the transferred part of the staging buffer would show."""
+    import torch
+    import paper_1501_03869_b200 as pat
+    g = _geom(900, 12, 2048)
+    rng = np.random.default_rng(31)
+    tau = (rng.uniform(lo_u, hi_u, size=(12, 900)) / FS).astype(np.float32)
+    tau[0, 0], tau[11, 899] = np.float32(lo_u / FS), np.float32(hi_u / FS)
+    tau[3, 5] = np.nan                                               # invalid entries do not widen the window
+    tau[4, 6] = np.float32(5000.0 / FS)
+    grid = pat.PatGrid.make(g.n, g.h, g.origin)
+    nbytes = pat.pat_plan_workspace_bytes(grid, 12, 900, 2048, 2)
+    ws = torch.full((nbytes + 256,), 0xFF, dtype=torch.uint8, device="cuda")
+    addr = (ws.data_ptr() + 255) // 256 * 256
+    h = pat.pat_plan_create(grid, None, g.sensors, 12, g.roi_index, 900, 2048, FS, 0.0, pat.PAT_W_PAPER, 2, addr, nbytes)
+    try:
+        pat.pat_set_travel_times(h, tau, 0, 12)
+        u = (tau * np.float32(FS)).astype(np.float32)
+        ok = (u >= 0) & (u < 2047)
+        k = np.floor(u[ok]).astype(np.int64)
+        first, count = pat.pat_get_trace_window(h)
+        assert (first, count) == expect
+        if count < 2048:
+            assert first <= max(0, k.min() - 1) and first + count >= min(2048, k.max() + 3)
+        for q in range(3):                                           # both staging buffers
+            tr = rng.standard_normal((2, 12, 2048)).astype(np.float32)
+            t = torch.from_numpy(tr).pin_memory()
+            im = torch.empty((2, 900), dtype=torch.float32).pin_memory()
+            pat.pat_backproject(h, t, im, 2)
+            torch.cuda.synchronize()
+            assert np.all(np.isfinite(im.numpy()))
+            assert_parity(im.numpy(), oracle.backproject(tau, tr, FS, 0.0, 1), "windowed H2D, call %d" % q)
+    finally:
+        pat.pat_destroy(h)
