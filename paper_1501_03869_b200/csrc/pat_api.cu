@@ -440,6 +440,8 @@ extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, cons
     p->use_pdl = !(env && env[0] == '1');
     env = std::getenv("PAT_FULL_H2D");                     // A/B switch: always transfer whole traces
     p->window_h2d = !(env && env[0] == '1');
+    env = std::getenv("PAT_FULL_PREPASS");                 // A/B switch: weight every sample of every trace
+    p->window_prepass = !(env && env[0] == '1');
 
     std::vector<int32_t> perm;
     try {
@@ -660,7 +662,9 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
         return PAT_OK;
     }
     if (p->profiling != 2) {
-        e = pat_launch_prepass(ctx, d_tr, bw, d_img, d.nsens, d.nt, p->nt4, nframes, bp, d.npix, p->wp, p->wd, t0fs, p->exact);
+        e = pat_launch_prepass(ctx, d_tr, bw, d_img, d.nsens, d.nt, p->nt4, nframes, bp, d.npix, p->wp, p->wd, t0fs, p->exact,
+                               p->window_prepass ? (conventional ? p->onfly_lo : p->need_lo) : 0,
+                               p->window_prepass ? (conventional ? p->onfly_hi : p->need_hi) : INT32_MAX);
         if (e) return cuda_fail(p, e, "pre-pass launch");
         ++p->launches;
     }

@@ -84,6 +84,7 @@ struct pat_plan {
     int num_sms = 0;
     int tune_wr = 0, tune_R = 0, tune_stages = 0;   // pat_set_gather_tuning overrides (0 = automatic)
     bool use_pdl = true;
+    bool window_prepass = true;       // H1 only over the samples the table can touch (PAT_FULL_PREPASS=1: all)
     bool window_h2d = true;           // host traces: copy only the samples the table can touch (PAT_FULL_H2D=1: all)
     std::vector<uint8_t> row_set;     // per sensor: tau row uploaded?
     int64_t rows_set = 0;
@@ -142,7 +143,8 @@ int pat_launch_row_meta(const PatLaunchCtx &ctx, const float *u_t, void *meta, i
 // exact (PAT_W_*_EXACT): bp counts CHANNELS, frame f owns channels 2f = wp*p[n] and 2f+1 = -wd*D[n].
 int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, float *images,
                        int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp,
-                       int64_t npix, float wp, float wd, float t0fs, bool exact = false);
+                       int64_t npix, float wp, float wd, float t0fs, bool exact = false,
+                       int32_t n_lo = 0, int32_t n_hi = INT32_MAX);   // only samples [n_lo, n_hi) of b are needed
 
 // Measurement only (pat_set_profiling mode 4): stream a_bytes + c_bytes in, nout floats out.
 int pat_launch_stream_probe(const PatLaunchCtx &ctx, const void *a, int64_t a_bytes, const void *c, int64_t c_bytes,

@@ -94,10 +94,10 @@ constexpr int kPreNs = 128;                                // samples per block
 __global__ void __launch_bounds__(256)
 prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
                int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int64_t npix, float wp, float wd,
-               float t0fs) {
+               float t0fs, int32_t n_lo) {
     asm volatile("griddepcontrol.launch_dependents;");
     __shared__ float out[kPreNs * 33];
-    const int32_t s = blockIdx.y, grp = blockIdx.z, n_begin = blockIdx.x * kPreNs;
+    const int32_t s = blockIdx.y, grp = blockIdx.z, n_begin = n_lo + blockIdx.x * kPreNs;
     {
         const int64_t nblk = (int64_t)gridDim.x * gridDim.y * gridDim.z;
         const int64_t blk = ((int64_t)grp * gridDim.y + s) * gridDim.x + blockIdx.x;
@@ -157,10 +157,10 @@ prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *_
 __global__ void __launch_bounds__(256)
 prepass_blocked_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
                        int32_t nsens, int32_t nt, int32_t ntb, int32_t nframes, int32_t log2_bp,
-                       int64_t npix, float wp, float wd, float t0fs) {
+                       int64_t npix, float wp, float wd, float t0fs, int32_t n_lo, int32_t quads) {
     asm volatile("griddepcontrol.launch_dependents;");
-    // grid = (quads of a row / 256, sensor, frame slot of the padded groups)
-    const int32_t s = blockIdx.y, f = blockIdx.z, bp = 1 << log2_bp, quads = ntb * 8;
+    // grid = (quads of the needed part of a row / 256, sensor, frame slot of the padded groups)
+    const int32_t s = blockIdx.y, f = blockIdx.z, bp = 1 << log2_bp;
     {
         const int64_t nblk = (int64_t)gridDim.x * gridDim.y * gridDim.z;
         const int64_t blk = ((int64_t)f * gridDim.y + s) * gridDim.x + blockIdx.x;
@@ -170,7 +170,7 @@ prepass_blocked_kernel(const float *__restrict__ traces, float *__restrict__ b, 
     }
     const int32_t q = blockIdx.x * 256 + threadIdx.x;
     if (q >= quads) return;
-    const int32_t n0 = q << 2;
+    const int32_t n0 = n_lo + (q << 2);
     float4 o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     if (f < nframes && quad_interior(n0, nt, wd)) {
         float w[6];
@@ -195,13 +195,12 @@ template <int BP>
 __global__ void __launch_bounds__(256)
 prepass_small_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
                      int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int64_t npix, float wp, float wd,
-                     float t0fs) {
+                     float t0fs, int32_t n_lo, int32_t quads) {
     asm volatile("griddepcontrol.launch_dependents;");
     const int64_t gid = (int64_t)blockIdx.x * 256 + threadIdx.x, nthr = (int64_t)gridDim.x * 256;
     for (int64_t q = gid; q < npix * nframes; q += nthr) images[q] = 0.0f;
-    const int32_t quads = nt4 >> 2;
     for (int64_t q = gid; q < (int64_t)nsens * quads; q += nthr) {
-        const int32_t s = (int32_t)(q / quads), n0 = (int32_t)(q - (int64_t)s * quads) << 2;
+        const int32_t s = (int32_t)(q / quads), n0 = n_lo + ((int32_t)(q - (int64_t)s * quads) << 2);
         float o[4][BP];
 #pragma unroll
         for (int f = 0; f < BP; ++f) {
@@ -244,7 +243,7 @@ template <int LAYOUT>
 __global__ void __launch_bounds__(256)
 prepass_exact_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
                      int32_t nsens, int32_t nt, int32_t nt4, int32_t ntb, int32_t nframes, int32_t log2_bp,
-                     int64_t npix, float wp, float wd) {
+                     int64_t npix, float wp, float wd, int32_t n_lo, int32_t quads) {
     asm volatile("griddepcontrol.launch_dependents;");
     {
         const int64_t nblk = (int64_t)gridDim.x * gridDim.y * gridDim.z;
@@ -257,9 +256,8 @@ prepass_exact_kernel(const float *__restrict__ traces, float *__restrict__ b, fl
     int32_t f, q;
     if (LAYOUT == 2) { f = blockIdx.z * 16 + (threadIdx.x & 15); q = blockIdx.x * 16 + (threadIdx.x >> 4); }
     else             { f = blockIdx.z; q = blockIdx.x * 256 + threadIdx.x; }
-    const int32_t quads = LAYOUT == 1 ? ntb * 8 : nt4 >> 2;
     if (q >= quads) return;
-    const int32_t n0 = q << 2;
+    const int32_t n0 = n_lo + (q << 2);
     float pv[4] = {0.0f, 0.0f, 0.0f, 0.0f}, dv[4] = {0.0f, 0.0f, 0.0f, 0.0f};
     if (f < nframes && n0 < nt) {
         float w[6];
@@ -346,48 +344,57 @@ int pat_launch_retile(const PatLaunchCtx &ctx, const float *src, float *u_t, con
 
 int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, float *images,
                        int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp,
-                       int64_t npix, float wp, float wd, float t0fs, bool exact) {
+                       int64_t npix, float wp, float wd, float t0fs, bool exact, int32_t n_lo, int32_t n_hi) {
+    // Only samples [n_lo, n_hi) of b can be read by a valid pixel (the caller's k-ranges; whole quads): the rest
+    // of b is left as it is.  The blocked layout works in whole 32-sample blocks.
+    const int32_t ntb = (nt + 31) / 32;
+    cudaStream_t st = (cudaStream_t)ctx.stream;
+    if (n_hi > nt4) n_hi = nt4;
+    if (n_lo < 0 || n_lo >= n_hi) { n_lo = 0; n_hi = 4; }           // nothing needed: still zero the images
+    n_lo &= ~3;
+    const bool blocked = pat_gather_blocked(bp);
+    if (blocked) { n_lo &= ~31; n_hi = (n_hi + 31) & ~31; if (n_hi > ntb * 32) n_hi = ntb * 32; }
+    const int32_t quads = (n_hi - n_lo + 3) >> 2;
     if (exact) {                                   // bp counts channels, two per frame
         if (bp < 2 || bp > 32) return (int)cudaErrorInvalidValue;
         int log2_bp = 0;
         while ((1 << log2_bp) < bp) ++log2_bp;
-        const int32_t fpg = bp / 2, groups = (nframes + fpg - 1) / fpg, ntb = (nt + 31) / 32;
-        cudaStream_t st = (cudaStream_t)ctx.stream;
+        const int32_t fpg = bp / 2, groups = (nframes + fpg - 1) / fpg;
         if (bp == 2) {
-            dim3 grid((unsigned)(((nt4 >> 2) + 255) / 256), (unsigned)nsens, (unsigned)groups);
-            prepass_exact_kernel<0><<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd);
-        } else if (pat_gather_blocked(bp)) {
-            dim3 grid((unsigned)((ntb * 8 + 255) / 256), (unsigned)nsens, (unsigned)(groups * fpg));
-            prepass_exact_kernel<1><<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd);
+            dim3 grid((unsigned)((quads + 255) / 256), (unsigned)nsens, (unsigned)groups);
+            prepass_exact_kernel<0><<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd, n_lo, quads);
+        } else if (blocked) {
+            dim3 grid((unsigned)((quads + 255) / 256), (unsigned)nsens, (unsigned)(groups * fpg));
+            prepass_exact_kernel<1><<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd, n_lo, quads);
         } else {
-            dim3 grid((unsigned)(((nt4 >> 2) + 15) / 16), (unsigned)nsens, (unsigned)groups);
-            prepass_exact_kernel<2><<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd);
+            dim3 grid((unsigned)((quads + 15) / 16), (unsigned)nsens, (unsigned)groups);
+            prepass_exact_kernel<2><<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd, n_lo, quads);
         }
         return (int)cudaGetLastError();
     }
     if (bp <= 2) {
-        const int64_t work = (int64_t)nsens * (nt4 >> 2);
+        const int64_t work = (int64_t)nsens * quads;
         int64_t blocks = (work + 255) / 256;
         if (blocks > (int64_t)ctx.num_sms * 16) blocks = (int64_t)ctx.num_sms * 16;
-        cudaStream_t st = (cudaStream_t)ctx.stream;
+        if (blocks < 1) blocks = 1;
         if (bp == 1)
-            prepass_small_kernel<1><<<(unsigned)blocks, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs);
+            prepass_small_kernel<1><<<(unsigned)blocks, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs, n_lo, quads);
         else
-            prepass_small_kernel<2><<<(unsigned)blocks, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs);
+            prepass_small_kernel<2><<<(unsigned)blocks, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs, n_lo, quads);
         return (int)cudaGetLastError();
     }
     int log2_bp = 0;
     while ((1 << log2_bp) < bp) ++log2_bp;
-    if (pat_gather_blocked(bp)) {
-        const int32_t groups = (nframes + bp - 1) / bp, ntb = (nt + 31) / 32;
-        dim3 grid((unsigned)((ntb * 8 + 255) / 256), (unsigned)nsens, (unsigned)(groups * bp));
-        prepass_blocked_kernel<<<grid, 256, 0, (cudaStream_t)ctx.stream>>>(traces, b, images, nsens, nt, ntb, nframes,
-                                                                          log2_bp, npix, wp, wd, t0fs);
+    if (blocked) {
+        const int32_t groups = (nframes + bp - 1) / bp;
+        dim3 grid((unsigned)((quads + 255) / 256), (unsigned)nsens, (unsigned)(groups * bp));
+        prepass_blocked_kernel<<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, ntb, nframes, log2_bp, npix, wp, wd, t0fs,
+                                                     n_lo, quads);
         return (int)cudaGetLastError();
     }
     if (bp != 32) return (int)cudaErrorInvalidValue;
     const int32_t groups = (nframes + bp - 1) / bp;
-    dim3 grid((unsigned)((nt4 + kPreNs - 1) / kPreNs), (unsigned)nsens, (unsigned)groups);
-    prepass_kernel<<<grid, 256, 0, (cudaStream_t)ctx.stream>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs);
+    dim3 grid((unsigned)((n_hi - n_lo + kPreNs - 1) / kPreNs), (unsigned)nsens, (unsigned)groups);
+    prepass_kernel<<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs, n_lo);
     return (int)cudaGetLastError();
 }
