@@ -151,7 +151,7 @@ prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *_
     }
 }
 
-// Bp = 4, 8, 16: the BLOCKED layout b[g][sensor][n/32][frame][32] (gather.cu, PPL == 3).  One thread per
+// Bp = 4, 8: the BLOCKED layout b[g][sensor][n/32][frame][32] (gather.cu, PPL == 3).  One thread per
 // (frame, sensor, 4 consecutive samples): reads straight from the traces (coalesced along time, the +-1
 // neighbours come from L1) and writes one 16-byte piece of a 128-byte block -- no transposition at all.
 __global__ void __launch_bounds__(256)
@@ -187,6 +187,42 @@ prepass_blocked_kernel(const float *__restrict__ traces, float *__restrict__ b, 
     const int32_t g = f >> log2_bp, fl = f & (bp - 1);
     float *dst = b + (((((int64_t)g * nsens + s) * ntb + (n0 >> 5)) << log2_bp) + fl) * 32 + (n0 & 31);
     *reinterpret_cast<float4 *>(dst) = o;
+}
+
+// Bp = 16 (interleaved [sensor][sample][16], gather.cu PPL == 4).  Thread = (frame, 4 consecutive samples) with
+// the 16 frames of the group as the fastest thread index: a half-warp writes the 64-byte line of one sample;
+// the two half-warps read the two 16-byte halves of the same 32-byte sector of every frame's row.
+__global__ void __launch_bounds__(256)
+prepass_il16_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
+                    int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int64_t npix, float wp, float wd,
+                    float t0fs, int32_t n_lo, int32_t quads) {
+    asm volatile("griddepcontrol.launch_dependents;");
+    {
+        const int64_t nblk = (int64_t)gridDim.x * gridDim.y * gridDim.z;
+        const int64_t blk = ((int64_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+        const int64_t tot = npix * nframes;
+        if (blk * 256 < tot)
+            for (int64_t q = blk * 256 + threadIdx.x; q < tot; q += nblk * 256) images[q] = 0.0f;
+    }
+    const int32_t s = blockIdx.y, grp = blockIdx.z, fl = threadIdx.x & 15, f = grp * 16 + fl;
+    const int32_t q = blockIdx.x * 16 + (threadIdx.x >> 4);
+    if (q >= quads) return;
+    const int32_t n0 = n_lo + (q << 2);
+    float4 o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    if (f < nframes && quad_interior(n0, nt, wd)) {
+        float w[6];
+        load_quad_interior(traces + ((int64_t)f * nsens + s) * nt, n0, w);
+        o = weight_quad_interior(w, n0, wp, t0fs);
+    } else if (f < nframes && n0 < nt) {
+        float w[6];
+        load_quad(traces + ((int64_t)f * nsens + s) * nt, n0, nt, w);
+        float *ov = reinterpret_cast<float *>(&o);
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (n0 + j < nt) ov[j] = weight_at(w + j, n0 + j, nt, wp, wd, t0fs);
+    }
+    float *dst = b + ((((int64_t)grp * nsens + s) * nt4 + n0) << 4) + fl;
+    dst[0] = o.x; dst[16] = o.y; dst[32] = o.z; dst[48] = o.w;
 }
 
 // Bp <= 2 (layout [sensor][sample][Bp]): one thread per 4 consecutive samples of all BP frames,
@@ -236,9 +272,9 @@ prepass_small_kernel(const float *__restrict__ traces, float *__restrict__ b, fl
 // of the channel count bp: channel 2f = wp*p_f[n], channel 2f+1 = -wd*D_f[n] (D as in weight_at; both
 // products are exact for wp = wd in {1, 2}).  One thread per (frame, sensor, 4 consecutive samples).
 //   LAYOUT 0  bp = 2   [sensor][sample][2]: a thread's 4 samples are 32 contiguous bytes
-//   LAYOUT 1  bp = 4, 8, 16 blocked [sensor][n/32][channel][32]: one 16-byte store per channel
-//   LAYOUT 2  bp = 32  [sensor][sample][32]: the 16 frames of a group are the fastest thread index, so that a
-//             half-warp writes the 128-byte line of one sample
+//   LAYOUT 1  bp = 4, 8 blocked [sensor][n/32][channel][32]: one 16-byte store per channel
+//   LAYOUT 2  bp = 16, 32  [sensor][sample][bp]: the bp/2 frames of a group are the fastest thread index, so that
+//             they write the line of one sample together
 template <int LAYOUT>
 __global__ void __launch_bounds__(256)
 prepass_exact_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
@@ -254,7 +290,11 @@ prepass_exact_kernel(const float *__restrict__ traces, float *__restrict__ b, fl
     }
     const int32_t s = blockIdx.y, bp = 1 << log2_bp;
     int32_t f, q;
-    if (LAYOUT == 2) { f = blockIdx.z * 16 + (threadIdx.x & 15); q = blockIdx.x * 16 + (threadIdx.x >> 4); }
+    if (LAYOUT == 2) {                                   // fpg = bp/2 frames of the group fastest
+        const int32_t lf = log2_bp - 1;
+        f = (blockIdx.z << lf) + (threadIdx.x & ((1 << lf) - 1));
+        q = blockIdx.x * (256 >> lf) + (threadIdx.x >> lf);
+    }
     else             { f = blockIdx.z; q = blockIdx.x * 256 + threadIdx.x; }
     if (q >= quads) return;
     const int32_t n0 = n_lo + (q << 2);
@@ -367,7 +407,8 @@ int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, f
             dim3 grid((unsigned)((quads + 255) / 256), (unsigned)nsens, (unsigned)(groups * fpg));
             prepass_exact_kernel<1><<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd, n_lo, quads);
         } else {
-            dim3 grid((unsigned)((quads + 15) / 16), (unsigned)nsens, (unsigned)groups);
+            const int32_t qpb = 256 / fpg;                 // quads per block
+            dim3 grid((unsigned)((quads + qpb - 1) / qpb), (unsigned)nsens, (unsigned)groups);
             prepass_exact_kernel<2><<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd, n_lo, quads);
         }
         return (int)cudaGetLastError();
@@ -390,6 +431,12 @@ int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, f
         dim3 grid((unsigned)((quads + 255) / 256), (unsigned)nsens, (unsigned)(groups * bp));
         prepass_blocked_kernel<<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, ntb, nframes, log2_bp, npix, wp, wd, t0fs,
                                                      n_lo, quads);
+        return (int)cudaGetLastError();
+    }
+    if (bp == 16) {
+        const int32_t groups = (nframes + 15) / 16;
+        dim3 grid((unsigned)((quads + 15) / 16), (unsigned)nsens, (unsigned)groups);
+        prepass_il16_kernel<<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs, n_lo, quads);
         return (int)cudaGetLastError();
     }
     if (bp != 32) return (int)cudaErrorInvalidValue;
