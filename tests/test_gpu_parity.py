@@ -109,3 +109,16 @@ def test_config4_shape_full_cube_analytic_tau_sampled_outputs():
     ref = oracle.backproject(np.ascontiguousarray(tau[:, pick]), tr, geom.fs, geom.t0, 1)
     assert_parity(got[:, pick], ref, "config4-shaped cube, sampled voxels")
     assert np.all(np.isfinite(got))
+
+
+@pytest.mark.parametrize("B", [12, 16])
+def test_config2_geometry_bp16_split_halves_path(B):
+    """The 9-16 frame class at the paper-scale geometry (the bench sweep's B = 16 row): interleaved [sample][16]
+    traces, a pixel's 8 lanes load one 128-byte run {b[k], b[k+1]} and the two halves meet at flush time."""
+    geom, tau = case(2)
+    tr = W.make_traces(geom, tau, frames=range(B))
+    ref = oracle.backproject(tau, tr, geom.fs, geom.t0, 1)
+    got = gpu_backproject(geom, tau, tr)
+    assert_parity(got, ref, "config2 geometry, %d frames" % B)
+    worst = max(errors(got[f], ref[f])[0] for f in range(B))
+    assert worst <= 1e-5
