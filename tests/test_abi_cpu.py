@@ -97,6 +97,11 @@ def test_null_plan_calls_are_safe():
     assert L.pat_backproject(None, None, None, 1, None) == pat.PAT_ERR_INVALID_ARG
     assert L.pat_set_travel_times(None, None, 0, 1, None) == pat.PAT_ERR_INVALID_ARG
     assert pat.pat_kernel_launches(None) == 0
+    assert L.pat_backproject_conventional(None, None, None, 1, 1500.0, None) == pat.PAT_ERR_INVALID_ARG
+    assert L.pat_set_pixel_weights(None, None, 0, 0, None) == pat.PAT_ERR_INVALID_ARG
+    assert L.pat_compute_solid_angle_weights(None, None, None) == pat.PAT_ERR_INVALID_ARG
+    assert L.pat_get_trace_window(None, None, None) == pat.PAT_ERR_INVALID_ARG
+    assert L.pat_set_roi_mask(None, None) == pat.PAT_ERR_INVALID_ARG
 
 
 def test_missing_library_raises_importerror(monkeypatch, tmp_path):
