@@ -189,9 +189,7 @@ prepass_blocked_kernel(const float *__restrict__ traces, float *__restrict__ b, 
     *reinterpret_cast<float4 *>(dst) = o;
 }
 
-// Bp = 16 (interleaved [sensor][sample][16], gather.cu PPL == 4).  Thread = (frame, 4 consecutive samples) with
-// the 16 frames of the group as the fastest thread index: a half-warp writes the 64-byte line of one sample;
-// the two half-warps read the two 16-byte halves of the same 32-byte sector of every frame's row.
+// Bp = 16 (interleaved [sensor][sample][16], gather.cu PPL == 4).
 __global__ void __launch_bounds__(256)
 prepass_il16_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
                     int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int64_t npix, float wp, float wd,
@@ -204,25 +202,42 @@ prepass_il16_kernel(const float *__restrict__ traces, float *__restrict__ b, flo
         if (blk * 256 < tot)
             for (int64_t q = blk * 256 + threadIdx.x; q < tot; q += nblk * 256) images[q] = 0.0f;
     }
-    const int32_t s = blockIdx.y, grp = blockIdx.z, fl = threadIdx.x & 15, f = grp * 16 + fl;
-    const int32_t q = blockIdx.x * 16 + (threadIdx.x >> 4);
+    // thread = (4 consecutive samples, 4 consecutive frames): four independent 16-byte loads (a warp reads 128
+    // contiguous bytes of each of 4 frame rows), four 16-byte stores (4 lanes = the 64-byte line of one sample)
+    const int32_t s = blockIdx.y, grp = blockIdx.z, fq = (threadIdx.x & 3) << 2;
+    const int32_t q = blockIdx.x * 64 + (threadIdx.x >> 2);
     if (q >= quads) return;
     const int32_t n0 = n_lo + (q << 2);
-    float4 o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-    if (f < nframes && quad_interior(n0, nt, wd)) {
-        float w[6];
-        load_quad_interior(traces + ((int64_t)f * nsens + s) * nt, n0, w);
-        o = weight_quad_interior(w, n0, wp, t0fs);
-    } else if (f < nframes && n0 < nt) {
-        float w[6];
-        load_quad(traces + ((int64_t)f * nsens + s) * nt, n0, nt, w);
-        float *ov = reinterpret_cast<float *>(&o);
+    float o[4][4];                                         // [sample][frame]
 #pragma unroll
-        for (int j = 0; j < 4; ++j)
-            if (n0 + j < nt) ov[j] = weight_at(w + j, n0 + j, nt, wp, wd, t0fs);
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+        for (int ff = 0; ff < 4; ++ff) o[j][ff] = 0.0f;
+    const int32_t f0 = grp * 16 + fq;
+    if (f0 + 3 < nframes && quad_interior(n0, nt, wd)) {
+        float w[4][6];
+#pragma unroll
+        for (int ff = 0; ff < 4; ++ff) load_quad_interior(traces + ((int64_t)(f0 + ff) * nsens + s) * nt, n0, w[ff]);
+#pragma unroll
+        for (int ff = 0; ff < 4; ++ff) {
+            const float4 v = weight_quad_interior(w[ff], n0, wp, t0fs);
+            o[0][ff] = v.x; o[1][ff] = v.y; o[2][ff] = v.z; o[3][ff] = v.w;
+        }
+    } else if (n0 < nt) {
+#pragma unroll
+        for (int ff = 0; ff < 4; ++ff) {
+            if (f0 + ff >= nframes) continue;
+            float w[6];
+            load_quad(traces + ((int64_t)(f0 + ff) * nsens + s) * nt, n0, nt, w);
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (n0 + j < nt) o[j][ff] = weight_at(w + j, n0 + j, nt, wp, wd, t0fs);
+        }
     }
-    float *dst = b + ((((int64_t)grp * nsens + s) * nt4 + n0) << 4) + fl;
-    dst[0] = o.x; dst[16] = o.y; dst[32] = o.z; dst[48] = o.w;
+    float *dst = b + ((((int64_t)grp * nsens + s) * nt4 + n0) << 4) + fq;
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+        *reinterpret_cast<float4 *>(dst + j * 16) = make_float4(o[j][0], o[j][1], o[j][2], o[j][3]);
 }
 
 // Bp <= 2 (layout [sensor][sample][Bp]): one thread per 4 consecutive samples of all BP frames,
@@ -435,7 +450,7 @@ int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, f
     }
     if (bp == 16) {
         const int32_t groups = (nframes + 15) / 16;
-        dim3 grid((unsigned)((quads + 15) / 16), (unsigned)nsens, (unsigned)groups);
+        dim3 grid((unsigned)((quads + 63) / 64), (unsigned)nsens, (unsigned)groups);
         prepass_il16_kernel<<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs, n_lo, quads);
         return (int)cudaGetLastError();
     }
