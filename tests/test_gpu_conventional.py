@@ -111,3 +111,24 @@ def test_conventional_errors():
         assert ei.value.status == pat.PAT_ERR_BAD_STATE
     finally:
         bare.close()
+
+
+def test_conventional_host_buffers_transfer_only_the_reachable_samples():
+    """Pinned host traces with the conventional BP: the strided H2D copy covers the k-ranges computed from the
+    geometry for this c0 (a changed c0 moves the window); three calls, both staging buffers."""
+    import torch
+    geom = W.make_geometry(0)
+    rng = np.random.default_rng(17)
+    plan = _plan(geom, 2)
+    try:
+        for c0 in (1560.0, 2400.0, 1560.0):
+            traces = rng.standard_normal((2, geom.nsens, geom.nt)).astype(np.float32)
+            tau = oracle.tau_conventional(geom.n, geom.h, geom.origin, geom.sensors, geom.roi_index, c0)
+            ref = oracle.backproject(tau, traces, geom.fs, geom.t0, 1)
+            tr = torch.from_numpy(traces).pin_memory()
+            img = torch.empty((2, geom.npix), dtype=torch.float32).pin_memory()
+            plan.backproject_conventional(tr, img, c0, 2)
+            torch.cuda.synchronize()
+            assert_parity(img.numpy(), ref, "conventional, host buffers, c0=%g" % c0)
+    finally:
+        plan.close()
