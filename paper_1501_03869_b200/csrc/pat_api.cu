@@ -438,6 +438,8 @@ extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, cons
     p->ws = (char *)workspace;
     const char *env = std::getenv("PAT_NO_PDL");
     p->use_pdl = !(env && env[0] == '1');
+    env = std::getenv("PAT_XSTEP");
+    p->xstep = env && env[0] == '1';
     env = std::getenv("PAT_FULL_H2D");                     // A/B switch: always transfer whole traces
     p->window_h2d = !(env && env[0] == '1');
     env = std::getenv("PAT_FULL_PREPASS");                 // A/B switch: weight every sample of every trace
@@ -642,6 +644,7 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
     }
     const bool prof = p->profiling == 1 && p->prof_events.size() < 3u * 65536u;
     PatLaunchCtx ctx{stream, p->num_sms, p->use_pdl && !prof};
+    ctx.xstep = p->xstep && ctx.use_pdl && p->profiling == 0;
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
     if (prof) {
         for (int q = 0; q < 3; ++q) {

@@ -84,6 +84,7 @@ struct pat_plan {
     int num_sms = 0;
     int tune_wr = 0, tune_R = 0, tune_stages = 0;   // pat_set_gather_tuning overrides (0 = automatic)
     bool use_pdl = true;
+    bool xstep = false;               // PAT_XSTEP=1 (measurement only, see PatLaunchCtx)
     bool window_prepass = true;       // H1 only over the samples the table can touch (PAT_FULL_PREPASS=1: all)
     bool window_h2d = true;           // host traces: copy only the samples the table can touch (PAT_FULL_H2D=1: all)
     std::vector<uint8_t> row_set;     // per sensor: tau row uploaded?
@@ -126,6 +127,10 @@ struct PatLaunchCtx {
     void *stream;
     int num_sms;
     bool use_pdl;
+    // PAT_XSTEP=1, MEASUREMENT ONLY: the gather releases its dependents at once and the B = 1
+    // pre-pass is launched programmatically without waiting, so the next step's pre-pass and gather prologue run under
+    // this gather's tail.  Only valid when consecutive calls use different plans and image buffers (bench.py's rotation).
+    bool xstep = false;
 };
 
 // tau rows [sensor_begin, +count) from src[count][npix] (device) -> u_t (tile-major, u = (tau-t0)*fs).

@@ -433,6 +433,19 @@ int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, f
         int64_t blocks = (work + 255) / 256;
         if (blocks > (int64_t)ctx.num_sms * 16) blocks = (int64_t)ctx.num_sms * 16;
         if (blocks < 1) blocks = 1;
+        if (bp == 1 && ctx.xstep) {                 // measurement only: programmatic launch, no wait in the kernel
+            cudaLaunchConfig_t cfg{};
+            cfg.gridDim = dim3((unsigned)blocks);
+            cfg.blockDim = dim3(256);
+            cfg.stream = st;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            attr[0].val.programmaticStreamSerializationAllowed = 1;
+            cfg.attrs = attr;
+            cfg.numAttrs = 1;
+            return (int)cudaLaunchKernelEx(&cfg, prepass_small_kernel<1>, traces, b, images, nsens, nt, nt4, nframes, npix,
+                                           wp, wd, t0fs, n_lo, quads);
+        }
         if (bp == 1)
             prepass_small_kernel<1><<<(unsigned)blocks, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs, n_lo, quads);
         else
