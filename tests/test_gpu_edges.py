@@ -319,3 +319,34 @@ def test_host_calls_transfer_only_the_samples_the_table_can_touch(lo_u, hi_u, ex
             assert_parity(im.numpy(), oracle.backproject(tau, tr, FS, 0.0, 1), "windowed H2D, call %d" % q)
     finally:
         pat.pat_destroy(h)
+
+
+def test_back_to_back_single_frame_calls_on_one_plan():
+    """One plan, 12 device calls without a synchronise in between: image buffers alternating between three tensors,
+    then the same tensor three times, different traces every call; every image must be the one of its own traces
+    (the weighted-trace buffer and the images are reused by the next call's pre-pass: stream order must hold)."""
+    import torch
+    import paper_1501_03869_b200 as pat
+    mode = "default"
+    geom, tau = case(1)
+    rng = np.random.default_rng(77)
+    plan = pat.Plan(geom.n, geom.h, geom.origin, None, geom.sensors, geom.roi_index, geom.nt, geom.fs, geom.t0, max_batch=1)
+    try:
+        plan.set_travel_times(tau)
+        ncall = 12
+        trs = [torch.from_numpy(rng.standard_normal((1, geom.nsens, geom.nt)).astype(np.float32)).cuda() for _ in range(ncall)]
+        ring = [torch.full((1, geom.npix), float("nan"), dtype=torch.float32, device="cuda") for _ in range(3)]
+        outs = []
+        st = torch.cuda.Stream()
+        torch.cuda.synchronize()
+        with torch.cuda.stream(st):
+            for q in range(ncall):
+                img = ring[q % 3] if q < 9 else ring[0]
+                plan.backproject(trs[q], img, 1, st)
+                outs.append(img.clone())                       # stream-ordered copy of this call's result
+        st.synchronize()
+        for q in (0, 1, 5, 8, 9, 10, 11):
+            ref = oracle.backproject(tau, trs[q].cpu().numpy(), geom.fs, geom.t0, 1)
+            assert_parity(outs[q].cpu().numpy(), ref, "back-to-back call %d, PAT_XSTEP=%s" % (q, mode))
+    finally:
+        plan.close()
