@@ -195,6 +195,10 @@ pat_status pat_get_trace_window(const pat_plan *plan, int32_t *first, int32_t *c
 /* Number of kernels of this library launched through `plan` so far (monotone counter). */
 int64_t pat_kernel_launches(const pat_plan *plan);
 
+/* Number of pat_backproject / pat_backproject_conventional calls on `plan` whose pre-pass was chained behind the
+ * previous call's gather with a programmatic edge (see pat_backproject, "Consecutive calls"). */
+int64_t pat_chained_calls(const pat_plan *plan);
+
 /* Override the gather's shared-memory geometry (tuning / test hook; 0 = choose automatically):
  *   wr      longest trace window one (tile, sensor) row may occupy in shared memory, a power of two in
  *           [8, 4096] (clipped to the frame-count class's limit): a row whose pixels span more than

@@ -73,6 +73,8 @@ def lib():
     L.pat_last_error.argtypes = [vp]
     L.pat_kernel_launches.restype = i64
     L.pat_kernel_launches.argtypes = [vp]
+    L.pat_chained_calls.restype = i64
+    L.pat_chained_calls.argtypes = [vp]
     L.pat_set_gather_tuning.restype = ctypes.c_int
     L.pat_set_gather_tuning.argtypes = [vp, i32, i32, i32]
     L.pat_set_profiling.restype = ctypes.c_int
@@ -210,6 +212,11 @@ def pat_kernel_launches(plan):
     return int(lib().pat_kernel_launches(plan))
 
 
+def pat_chained_calls(plan):
+    """Calls whose pre-pass was chained behind the previous call's gather (cross-call overlap inside a capture)."""
+    return int(lib().pat_chained_calls(plan))
+
+
 def pat_set_gather_tuning(plan, wr=0, rows=0, stages=0):
     return _check(plan, lib().pat_set_gather_tuning(plan, wr, rows, stages))
 
@@ -315,6 +322,9 @@ class Plan:
 
     def launches(self):
         return pat_kernel_launches(self.handle)
+
+    def chained_calls(self):
+        return pat_chained_calls(self.handle)
 
     def close(self):
         if getattr(self, "handle", None):

@@ -5,16 +5,137 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <numeric>
 
 namespace {
 
-std::string g_create_error;            // last pat_plan_create failure (plan == NULL in pat_last_error)
+thread_local std::string g_create_error;   // last pat_plan_create failure of THIS thread (plan == NULL in pat_last_error)
+
+// ---- cross-call overlap: the launch chain ------------------------------------------------------------------
+// One frame of configs[1] is ~10 us of GPU work: between two calls the launch gap, the gather's prologue and the
+// ragged end of its CTAs are a third of that.  Inside a stream capture (CUDA graph) consecutive calls are therefore
+// NOT captured as one linear chain.  With P_j / G_j the pre-pass / gather node of call j of an uninterrupted run
+// of calls on the capturing stream, the edges are
+//     G_{j-1} --programmatic--> G_j    the CTAs of G_j take the SM slots the CTAs of G_{j-1} free one by one, and
+//                                      stream the table beside the draining G_{j-1};
+//     P_j     --full----------> G_j    b (and the zeroed images) are complete before G_j starts;
+//     G_{j-3}, P_{j-1} --full-> P_j    and NO edge from G_{j-1}, G_{j-2}: the pre-pass of call j runs while the two
+//                                      gathers before it are still busy, so its latency (a trip to HBM behind the table
+//                                      stream, ~4 us) is off the critical path.  (The edge from P_{j-1} keeps the
+//                                      pre-passes one ordered chain, which is how the graph executor runs them early.)
+// What makes that safe is carried by those edges alone:
+//   * b is triple-buffered per plan (calls rotate through three buffers): P_j writes the buffer G_{j-3} read, and
+//     G_{j-3} has completed; G_{j-1} and G_{j-2} read the other two;
+//   * G_j needs P_j, hence G_{j-3}: at most three gathers of a run are ever in flight, and they only READ shared
+//     data (table, work list) and accumulate into their own images;
+//   * the host allows the edges only if nothing foreign sits between the calls -- the capture's dependency set at
+//     call j is exactly {G_{j-1}} -- and if the images and traces of call j do not overlap the images of call j-1
+//     (P_j zeroes them while that gather may still accumulate); if they overlap those of call j-2 (a caller
+//     alternating between two image buffers), P_j hangs on G_{j-2} instead of G_{j-3}.  Everything enqueued before
+//     the run is ordered before P_0, hence before every node of the run; whatever is captured after call j depends
+//     on G_j, and one thread of every gather executes griddepcontrol.wait before the grid finishes, so the
+//     completion of G_j implies the completion of G_{j-1} (and so on down the run).
+// Any other call -- outside a capture, host buffers, overlapping images, foreign work in between -- is captured /
+// launched the ordinary way (P then G in stream order, G's prologue overlapping P through a programmatic launch).
+struct ChainCall {
+    cudaGraphNode_t gather;
+    uintptr_t img_lo, img_hi;
+};
+struct ChainRun {
+    unsigned long long capture_id = 0;
+    cudaGraphNode_t head_prepass = nullptr;     // P_{j-1}: the latest pre-pass of the run (P_j hangs on it as well,
+                                                // which keeps the pre-passes one ordered chain beside the gathers)
+    std::vector<ChainCall> calls;               // the last (up to) three calls of the run, oldest first
+};
+std::mutex g_chain_mu;
+std::vector<ChainRun> g_chain;            // one entry per capture in progress (bounded, oldest dropped)
+
+bool capture_deps(cudaStream_t st, unsigned long long *id, cudaGraphNode_t *node) {
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    const cudaGraphNode_t *deps = nullptr;
+    const cudaGraphEdgeData *edges = nullptr;
+    size_t nd = 0;
+    if (cudaStreamGetCaptureInfo_v3(st, &cs, id, nullptr, &deps, &edges, &nd) != cudaSuccess) { cudaGetLastError(); return false; }
+    if (cs != cudaStreamCaptureStatusActive) { *id = 0; return false; }
+    if (nd != 1 || !deps) return false;
+    *node = deps[0];
+    return true;
+}
+
+ChainRun *find_run(unsigned long long id) {
+    for (ChainRun &r : g_chain)
+        if (r.capture_id == id) return &r;
+    return nullptr;
+}
+
+// Decision for the call about to be captured.  chained: the node P_j must depend on (pre_dep) and G_{j-1}.
+struct ChainPlan {
+    bool chained = false;
+    unsigned long long capture_id = 0;
+    cudaGraphNode_t pre_dep = nullptr, prev_gather = nullptr, bound_dep = nullptr;   // bound_dep: G_{j-3} or NULL
+};
+ChainPlan chain_begin(cudaStream_t st, const void *traces, size_t tbytes, const void *images, size_t ibytes, int depth) {
+    ChainPlan cp;
+    cudaGraphNode_t node = nullptr;
+    const bool single = capture_deps(st, &cp.capture_id, &node);
+    if (!cp.capture_id) return cp;                                // not capturing
+    std::lock_guard<std::mutex> lk(g_chain_mu);
+    ChainRun *r = find_run(cp.capture_id);
+    if (!single || !r || r->calls.empty() || r->calls.back().gather != node) return cp;
+    const uintptr_t i0 = (uintptr_t)images, i1 = i0 + ibytes, t0 = (uintptr_t)traces, t1 = t0 + tbytes;
+    const size_t n = r->calls.size();
+    auto clash = [&](const ChainCall &c) {
+        return !(i1 <= c.img_lo || c.img_hi <= i0) || !(t1 <= c.img_lo || c.img_hi <= t0);
+    };
+    if (clash(r->calls[n - 1])) return cp;                        // G_{j-1} will still be running: ordinary capture
+    cp.chained = true;
+    cp.prev_gather = node;
+    // images alternating between two buffers (A, B, A, ...): P_j zeroes what G_{j-2} wrote, so it waits for that one
+    if (n >= 2 && (depth <= 2 || clash(r->calls[n - 2]))) cp.bound_dep = r->calls[n - 2].gather;
+    else cp.bound_dep = n >= 3 ? r->calls[n - 3].gather : nullptr;
+    cp.pre_dep = r->head_prepass;
+    return cp;
+}
+
+// After the launches of a call inside a capture: extend the run, or start a new one at this call.
+void chain_commit(const ChainPlan &cp, cudaGraphNode_t prepass, cudaGraphNode_t gather, const void *images, size_t ibytes) {
+    if (!cp.capture_id) return;
+    std::lock_guard<std::mutex> lk(g_chain_mu);
+    ChainRun *r = find_run(cp.capture_id);
+    if (!r) {
+        if (g_chain.size() >= 16) g_chain.erase(g_chain.begin());
+        g_chain.emplace_back();
+        r = &g_chain.back();
+        r->capture_id = cp.capture_id;
+    }
+    if (!cp.chained) r->calls.clear();
+    r->head_prepass = prepass;
+    if (!gather || !r->head_prepass) { r->calls.clear(); r->head_prepass = nullptr; return; }   // nothing to chain behind
+    r->calls.push_back(ChainCall{gather, (uintptr_t)images, (uintptr_t)images + ibytes});
+    if (r->calls.size() > 3) r->calls.erase(r->calls.begin());
+}
+
+cudaError_t set_capture_deps(cudaStream_t st, cudaGraphNode_t full_a, cudaGraphNode_t full_b, cudaGraphNode_t programmatic) {
+    cudaGraphNode_t nodes[3];
+    cudaGraphEdgeData edges[3];
+    std::memset(edges, 0, sizeof(edges));
+    size_t n = 0;
+    if (full_a) nodes[n++] = full_a;
+    if (full_b && full_b != full_a) nodes[n++] = full_b;
+    if (programmatic) {
+        edges[n].from_port = cudaGraphKernelNodePortProgrammatic;
+        edges[n].type = cudaGraphDependencyTypeProgrammatic;
+        nodes[n++] = programmatic;
+    }
+    return cudaStreamUpdateCaptureDependencies_v2(st, nodes, edges, n, cudaStreamSetCaptureDependencies);
+}
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -147,10 +268,8 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
     std::vector<Entry> list;
     std::vector<int32_t> cta_chunk;
     std::vector<int32_t> cost;                       // per chunk: fixed part + slots
-    int32_t chunk_cost = 6;
-    if (const char *cc = std::getenv("PAT_CHUNK_COST")) chunk_cost = std::max(0, std::atoi(cc));
-    int32_t slow_cost = 5;                           // a slot of a checked chunk, in units of half a fast slot
-    if (const char *cc = std::getenv("PAT_SLOW_COST")) slow_cost = std::max(1, std::atoi(cc));
+    const int32_t chunk_cost = p->env.chunk_cost;
+    const int32_t slow_cost = p->env.slow_cost;      // a slot of a checked chunk, in units of half a fast slot
     const size_t per_chunk = (size_t)R + 1;
     try {
         list.reserve((size_t)(V / R + ntiles + 16) * per_chunk);
@@ -238,8 +357,8 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
     } catch (...) { return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
     if (list.size() / per_chunk > (size_t)INT32_MAX) return fail(p, PAT_ERR_UNSUPPORTED, "work list too long");
     sc.nchunks = (int64_t)(list.size() / per_chunk);
-    if (const char *fn = std::getenv("PAT_SCHED_DUMP")) {        // diagnostic: per-CTA share composition
-        if (FILE *f = std::fopen(fn, "w")) {
+    if (!p->env.sched_dump.empty()) {                            // diagnostic: per-CTA share composition
+        if (FILE *f = std::fopen(p->env.sched_dump.c_str(), "w")) {
             for (int64_t c = 0; c < G; ++c) {
                 int64_t nch = cta_chunk[c + 1] - cta_chunk[c], nsl = 0, nwin = 0, nfast = 0;
                 for (int64_t q = cta_chunk[c]; q < cta_chunk[c + 1]; ++q) {
@@ -255,8 +374,8 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
             std::fclose(f);
         }
     }
-    if (const char *dbg = std::getenv("PAT_DEBUG")) {
-        if (dbg[0] == '1') {
+    {
+        if (p->env.debug) {
             int64_t ns = 0, nc = 0, nreal = 0;
             for (size_t q = 0; q < list.size(); q += per_chunk) {
                 ns += list[q].z & 1; nc += (list[q].z >> 1) & 1; nreal += list[q].z >> 8;
@@ -286,7 +405,7 @@ pat_status get_schedule(pat_plan *p, int bp, bool onfly, PatSchedule **out) {
     for (PatSchedule &sc : p->schedules)
         if (sc.cfg.bp == bp && sc.cfg.onfly == onfly) { *out = &sc; return PAT_OK; }
     PatGatherConfig cfg = pat_gather_config(bp, p->tune_wr, p->tune_R, p->tune_stages, onfly, p->exact,
-                                            p->d_w_t != nullptr);
+                                            p->d_w_t != nullptr, p->env);
     return build_schedule(p, cfg, out);
 }
 
@@ -363,6 +482,9 @@ PatLayout pat_layout(const PatDims &d) {
     const int bp = pat_frames_per_group(d.max_batch);
     const size_t padded = (size_t)(d.max_batch + bp - 1) / bp * bp;
     L.bd = take(padded * d.nsens * ((d.nt + 31) / 32 * 32) * sizeof(float));
+    L.bd2 = take(padded * d.nsens * ((d.nt + 31) / 32 * 32) * sizeof(float));
+    L.bd3 = take(padded * d.nsens * ((d.nt + 31) / 32 * 32) * sizeof(float));
+    L.sync = take(768);
     L.perm = take((size_t)d.ntiles * kTilePix * sizeof(int32_t));
     L.traces = take((size_t)d.max_batch * d.nsens * d.nt * sizeof(float));
     L.traces2 = take((size_t)d.max_batch * d.nsens * d.nt * sizeof(float));
@@ -438,8 +560,21 @@ extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, cons
     p->ws = (char *)workspace;
     const char *env = std::getenv("PAT_NO_PDL");
     p->use_pdl = !(env && env[0] == '1');
-    env = std::getenv("PAT_XSTEP");
-    p->xstep = env && env[0] == '1';
+    {   // tuning / diagnostic knobs: read here, once (PatTune)
+        auto env_int = [](const char *n, int dflt) { const char *v = std::getenv(n); return v ? std::atoi(v) : dflt; };
+        p->env.wr = env_int("PAT_WR", 0); p->env.R = env_int("PAT_R", 0); p->env.stages = env_int("PAT_STAGES", 0);
+        p->env.cap = env_int("PAT_CAP", 0); p->env.budget_kb = env_int("PAT_BUDGET_KB", 0);
+        p->env.chunk_cost = std::max(0, env_int("PAT_CHUNK_COST", 6));
+        p->env.slow_cost = std::max(1, env_int("PAT_SLOW_COST", 5));
+        p->env.debug = env_int("PAT_DEBUG", 0) == 1;
+        p->env.chain_depth = env_int("PAT_CHAIN_DEPTH", 3);
+        if (const char *fn = std::getenv("PAT_SCHED_DUMP")) p->env.sched_dump = fn;
+    }
+    env = std::getenv("PAT_TRACE_FILE");                   // diagnostic: per-CTA timeline of the last gather launch
+    p->trace_file = env && env[0];
+    if (p->trace_file) p->trace_file_name = env;
+    env = std::getenv("PAT_ENABLE_PROBES");                // measurement modes of pat_set_profiling (bench.py)
+    p->probes = env && env[0] == '1';
     env = std::getenv("PAT_FULL_H2D");                     // A/B switch: always transfer whole traces
     p->window_h2d = !(env && env[0] == '1');
     env = std::getenv("PAT_FULL_PREPASS");                 // A/B switch: weight every sample of every trace
@@ -487,8 +622,13 @@ extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, cons
     }
     p->device = dev;
     p->num_sms = sms;
+    {
+        int lo = 0, hi = 0;
+        if (cudaDeviceGetStreamPriorityRange(&lo, &hi) == cudaSuccess) p->prio_high = hi; else cudaGetLastError();
+    }
     p->host_perm = perm;
     e = cudaMemcpy(p->ws + p->lay.perm, perm.data(), perm.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemset(p->ws + p->lay.sync, 0, 768);
     if (e != cudaSuccess) { delete p; return cuda_fail(nullptr, e, "upload of the pixel permutation"); }
     if (!(std::getenv("PAT_NO_PIPE") && std::getenv("PAT_NO_PIPE")[0] == '1')) {
         cudaStream_t cs = nullptr;
@@ -644,7 +784,15 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
     }
     const bool prof = p->profiling == 1 && p->prof_events.size() < 3u * 65536u;
     PatLaunchCtx ctx{stream, p->num_sms, p->use_pdl && !prof};
-    ctx.xstep = p->xstep && ctx.use_pdl && p->profiling == 0;
+    ctx.high_priority = p->prio_high;
+    const size_t ibytes = (size_t)nframes * d.npix * sizeof(float);
+    const bool do_gather = sc->grid_x > 0 && p->profiling != 3;
+    const bool do_pre = p->profiling != 2;
+    // launch chain (see the top of this file): only for device buffers inside a capture
+    ChainPlan cp;
+    if (ctx.use_pdl && td && p->profiling != 4)
+        cp = chain_begin(st, traces, (size_t)nframes * d.nsens * d.nt * sizeof(float), images, ibytes, p->env.chain_depth);
+    if (cp.chained && !do_gather) cp.chained = false;
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
     if (prof) {
         for (int q = 0; q < 3; ++q) {
@@ -654,9 +802,18 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
         }
         cudaEventRecord(ev[0], st);
     }
-    float *bw = (float *)(p->ws + p->lay.bd);
+    // consecutive calls rotate through the three b buffers and their counters
+    const int slot_b = p->b_slot;
+    p->b_slot = (p->b_slot + 1) % 3;
+    float *bw = (float *)(p->ws + (slot_b == 0 ? p->lay.bd : slot_b == 1 ? p->lay.bd2 : p->lay.bd3));
+    uint32_t *sync = (uint32_t *)(p->ws + p->lay.sync) + 64 * slot_b;
     const float t0fs = (float)((double)p->t0 * (double)p->fs);
     int e = 0;
+    if (p->sync_dirty) {              // an earlier call failed between its two launches: counters may be non-zero
+        cudaError_t ce = cudaMemsetAsync(p->ws + p->lay.sync, 0, 768, st);
+        if (ce != cudaSuccess) return cuda_fail(p, ce, "counter reset");
+        p->sync_dirty = false;
+    }
     if (p->profiling == 4) {          // measurement: the step's footprint (table + b in, images out) as a plain stream
         e = pat_launch_stream_probe(ctx, p->ws + p->lay.tau, (int64_t)d.ntiles * kTilePix * d.nsens * 4,
                                     bw, (int64_t)nch * d.nsens * p->nt4 * 4, d_img, (int64_t)nframes * d.npix);
@@ -664,30 +821,50 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
         ++p->launches;
         return PAT_OK;
     }
-    if (p->profiling != 2) {
+    if (do_gather && p->trace_file && !p->trace_dev && nframes <= 32) {   // diagnostic timeline (PAT_TRACE_FILE at create)
+        if (cudaMalloc((void **)&p->trace_dev, (size_t)(sc->grid_x + 1) * 8 * sizeof(unsigned long long)) == cudaSuccess) {
+            p->trace_ctas = sc->grid_x;
+            cudaMemset(p->trace_dev, 0, (size_t)(sc->grid_x + 1) * 8 * sizeof(unsigned long long));
+        } else {
+            p->trace_dev = nullptr;
+        }
+    }
+    if (p->trace_dev && p->trace_ctas == sc->grid_x) ctx.pre_trace = p->trace_dev + (size_t)sc->grid_x * 8;
+    cudaGraphNode_t node_pre = nullptr, node_gather = nullptr;
+    unsigned long long cid = 0;
+    if (do_pre) {
+        if (cp.chained) {             // P_j behind P_{j-1} and G_{j-3} only
+            cudaError_t ce = set_capture_deps(st, cp.pre_dep, cp.bound_dep, nullptr);
+            if (ce != cudaSuccess) return cuda_fail(p, ce, "capture dependencies (pre-pass)");
+        }
         e = pat_launch_prepass(ctx, d_tr, bw, d_img, d.nsens, d.nt, p->nt4, nframes, bp, d.npix, p->wp, p->wd, t0fs, p->exact,
                                p->window_prepass ? (conventional ? p->onfly_lo : p->need_lo) : 0,
-                               p->window_prepass ? (conventional ? p->onfly_hi : p->need_hi) : INT32_MAX);
+                               p->window_prepass ? (conventional ? p->onfly_hi : p->need_hi) : INT32_MAX,
+                               do_gather ? sync : nullptr);
         if (e) return cuda_fail(p, e, "pre-pass launch");
         ++p->launches;
+        if (cp.capture_id) capture_deps(st, &cid, &node_pre);
     }
     if (prof) cudaEventRecord(ev[1], st);
     if (piped) cudaEventRecord((cudaEvent_t)p->ev_read[slot], st);        // the staged traces have been consumed
-    if (sc->grid_x > 0 && p->profiling != 3) {
-        if (std::getenv("PAT_TRACE_FILE") && !p->trace_dev && nframes <= 32) {   // diagnostic timeline
-            if (cudaMalloc((void **)&p->trace_dev, (size_t)sc->grid_x * 8 * sizeof(unsigned long long)) == cudaSuccess)
-                p->trace_ctas = sc->grid_x;
-            else
-                p->trace_dev = nullptr;
+    if (do_gather) {
+        if (cp.chained) {             // G_j: full edges from P_j (and G_{j-3}), programmatic edge from G_{j-1}
+            cudaError_t ce = set_capture_deps(st, node_pre, do_pre ? nullptr : cp.bound_dep, cp.prev_gather);
+            if (ce != cudaSuccess) { p->sync_dirty = do_pre; return cuda_fail(p, ce, "capture dependencies (gather)"); }
+            ctx.use_pdl = false;      // the edges are explicit: no launch attribute
+            ++p->chained;
         }
         e = pat_launch_gather(ctx, sc->cfg, (const float *)(p->ws + p->lay.tau), bw, sc->d_sched, sc->d_cta_chunk,
                               sc->grid_x, p->d_perm_masked ? p->d_perm_masked : (const int32_t *)(p->ws + p->lay.perm),
                               d_img, d.nsens, d.npix, d.nt,
                               p->nt4, nframes, p->trace_ctas == sc->grid_x ? p->trace_dev : nullptr,
-                              conventional ? &onfly : nullptr, t0fs, p->d_w_t);
-        if (e) return cuda_fail(p, e, "gather launch");
+                              conventional ? &onfly : nullptr, t0fs, p->d_w_t,
+                              do_pre ? sync : nullptr);
+        if (e) { p->sync_dirty = do_pre; return cuda_fail(p, e, "gather launch"); }
         ++p->launches;
+        if (cp.capture_id) capture_deps(st, &cid, &node_gather);
     }
+    if (cp.capture_id && td) chain_commit(cp, do_pre ? node_pre : node_gather, node_gather, images, ibytes);
     if (prof) cudaEventRecord(ev[2], st);
     if (!td) {
         cudaError_t ce = cudaMemcpyAsync(images, d_img, (size_t)nframes * d.npix * sizeof(float),
@@ -704,11 +881,14 @@ static void drop_events(pat_plan *p) {
 
 extern "C" pat_status pat_destroy(pat_plan *p) {
     if (p && p->trace_dev) {                   // PAT_TRACE_FILE: dump the per-CTA timeline of the last launch
-        std::vector<unsigned long long> h((size_t)p->trace_ctas * 8);
+        std::vector<unsigned long long> h((size_t)(p->trace_ctas + 1) * 8);
         cudaDeviceSynchronize();
         if (cudaMemcpy(h.data(), p->trace_dev, h.size() * 8, cudaMemcpyDeviceToHost) == cudaSuccess)
-            if (const char *fn = std::getenv("PAT_TRACE_FILE"))
-                if (FILE *f = std::fopen(fn, "wb")) { std::fwrite(h.data(), 8, h.size(), f); std::fclose(f); }
+            if (p->trace_file) {                   // one file per plan: <name>.<k>, k counting the plans destroyed so far
+                static std::atomic<int> serial{0};
+                const std::string fn = p->trace_file_name + "." + std::to_string(serial.fetch_add(1));
+                if (FILE *f = std::fopen(fn.c_str(), "wb")) { std::fwrite(h.data(), 8, h.size(), f); std::fclose(f); }
+            }
         cudaFree(p->trace_dev);
     }
     if (p) {
@@ -730,6 +910,8 @@ extern "C" pat_status pat_destroy(pat_plan *p) {
 extern "C" pat_status pat_set_profiling(pat_plan *p, int32_t enable) {
     if (!p) return PAT_ERR_INVALID_ARG;
     if (enable < 0 || enable > 4) return fail(p, PAT_ERR_INVALID_ARG, "profiling mode must be 0..4");
+    if (enable >= 2 && !p->probes)
+        return fail(p, PAT_ERR_UNSUPPORTED, "modes 2-4 leave garbage images: measurement only, plan must be created with PAT_ENABLE_PROBES=1");
     p->profiling = enable;
     return PAT_OK;
 }
@@ -760,6 +942,8 @@ extern "C" const char *pat_last_error(const pat_plan *p) {
 }
 
 extern "C" int64_t pat_kernel_launches(const pat_plan *p) { return p ? p->launches : 0; }
+
+extern "C" int64_t pat_chained_calls(const pat_plan *p) { return p ? p->chained : 0; }
 
 extern "C" pat_status pat_get_trace_window(const pat_plan *p, int32_t *first, int32_t *count) {
     if (!p || !first || !count) return PAT_ERR_INVALID_ARG;

@@ -27,6 +27,9 @@ struct PatLayout {            // byte offsets into the caller's workspace
     size_t tau = 0;           // float  [ntiles][nsens][256]   u = fl32(fl32(tau - t0)*fs), tile-major
     size_t meta = 0;          // int2   [ntiles*nsens]         {kmin, kmax} of each row
     size_t bd = 0;            // float  weighted traces b: [g][nsens][nt4][Bp] (Bp <= 2) or blocked [g][nsens][ntb][Bp][32]
+    size_t bd2 = 0, bd3 = 0;  // float  two more b buffers: consecutive calls rotate, so the pre-pass of call j may run while
+                              //        the gathers of calls j-1 and j-2 still read theirs (cross-call overlap, pat_api.cu)
+    size_t sync = 0;          // uint32 [3][64] per b buffer: [0] pre-pass blocks done, [1] gather CTAs done, [32] b-ready flag
     size_t perm = 0;          // int32  [ntiles*256]  slot -> position in roi list, -1 = pad
     size_t traces = 0;        // float  [max_batch][nsens][nt]    staging for host traces
     size_t traces2 = 0;       // float  second staging buffer: the copy of call i+1 overlaps the kernels of call i
@@ -50,6 +53,17 @@ struct PatGatherConfig {
     bool onfly = false;       // work list of the conventional BP (k-ranges from the geometry, no table)
     bool exact = false;       // PAT_W_*_EXACT: the bp "frames" are channel pairs {wp*p, -wd*D} of bp/2 frames
     bool weighted = false;    // pat_set_pixel_weights: a stage holds R weight rows after its R u rows
+};
+
+// Tuning / diagnostic knobs, read from the environment ONCE, in pat_plan_create (never on a call path):
+// PAT_WR, PAT_R, PAT_STAGES, PAT_CAP, PAT_BUDGET_KB (shared-memory geometry), PAT_CHUNK_COST, PAT_SLOW_COST (cost
+// model of the work-list dealer), PAT_DEBUG=1 (schedule summary on stderr), PAT_SCHED_DUMP=<file>.
+struct PatTune {
+    int wr = 0, R = 0, stages = 0, cap = 0, budget_kb = 0;
+    int chunk_cost = 6, slow_cost = 5;
+    bool debug = false;
+    int chain_depth = 3;          // PAT_CHAIN_DEPTH (A/B): 3 = the pre-pass of call j hangs on the gather of call j-3, 2 = on j-2
+    std::string sched_dump;
 };
 
 // Conventional BP: tau = |r - s| / c0 computed inside the gather.
@@ -82,9 +96,13 @@ struct pat_plan {
     char *ws = nullptr;       // device workspace base (borrowed)
     int device = 0;
     int num_sms = 0;
+    int prio_high = 0;                // greatest stream priority of the device (cudaDeviceGetStreamPriorityRange)
     int tune_wr = 0, tune_R = 0, tune_stages = 0;   // pat_set_gather_tuning overrides (0 = automatic)
+    PatTune env;                                    // environment knobs as they were at pat_plan_create
     bool use_pdl = true;
-    bool xstep = false;               // PAT_XSTEP=1 (measurement only, see PatLaunchCtx)
+    bool probes = false;              // PAT_ENABLE_PROBES=1 at create: pat_set_profiling's kernel-only modes 2-4 allowed
+    int b_slot = 0;                   // which of the three b buffers the next call writes
+    bool sync_dirty = false;          // a launch failed between pre-pass and gather: re-zero the counters first
     bool window_prepass = true;       // H1 only over the samples the table can touch (PAT_FULL_PREPASS=1: all)
     bool window_h2d = true;           // host traces: copy only the samples the table can touch (PAT_FULL_H2D=1: all)
     std::vector<uint8_t> row_set;     // per sensor: tau row uploaded?
@@ -96,6 +114,9 @@ struct pat_plan {
     std::vector<float> sensors;
     std::vector<int64_t> roi;         // empty => all nodes
     int64_t launches = 0;
+    int64_t chained = 0;              // calls whose pre-pass was launched with a programmatic edge (launch chain)
+    bool trace_file = false;                   // PAT_TRACE_FILE was set at create
+    std::string trace_file_name;
     unsigned long long *trace_dev = nullptr;   // PAT_TRACE_FILE diagnostic: timeline of the last gather launch
     int trace_ctas = 0;
     // host-buffer calls: H2D on an own copy stream into alternating staging buffers, so that the transfer
@@ -127,10 +148,8 @@ struct PatLaunchCtx {
     void *stream;
     int num_sms;
     bool use_pdl;
-    // PAT_XSTEP=1, MEASUREMENT ONLY: the gather releases its dependents at once and the B = 1
-    // pre-pass is launched programmatically without waiting, so the next step's pre-pass and gather prologue run under
-    // this gather's tail.  Only valid when consecutive calls use different plans and image buffers (bench.py's rotation).
-    bool xstep = false;
+    unsigned long long *pre_trace = nullptr;   // PAT_TRACE_FILE diagnostic: {pre-pass block 0 start, flag raised}
+    int high_priority = 0;                     // the device's greatest stream priority (pre-pass launches)
 };
 
 // tau rows [sensor_begin, +count) from src[count][npix] (device) -> u_t (tile-major, u = (tau-t0)*fs).
@@ -149,7 +168,9 @@ int pat_launch_row_meta(const PatLaunchCtx &ctx, const float *u_t, void *meta, i
 int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, float *images,
                        int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp,
                        int64_t npix, float wp, float wd, float t0fs, bool exact = false,
-                       int32_t n_lo = 0, int32_t n_hi = INT32_MAX);   // only samples [n_lo, n_hi) of b are needed
+                       int32_t n_lo = 0, int32_t n_hi = INT32_MAX,    // only samples [n_lo, n_hi) of b are needed
+                       uint32_t *ready = nullptr);                    // [0]: every block counts itself when its part of b / images is
+                                                                      // written, the last one raises the flag [32]
 
 // Measurement only (pat_set_profiling mode 4): stream a_bytes + c_bytes in, nout floats out.
 int pat_launch_stream_probe(const PatLaunchCtx &ctx, const void *a, int64_t a_bytes, const void *c, int64_t c_bytes,
@@ -159,8 +180,8 @@ int pat_launch_stream_probe(const PatLaunchCtx &ctx, const void *a, int64_t a_by
 int pat_frames_per_group(int32_t nframes);
 bool pat_gather_blocked(int bp);       // trace layout [sensor][n/32][frame][32] instead of [sensor][n][frame]
 int pat_gather_wrmax(int bp);          // default / largest slot window for this frame-count class
-PatGatherConfig pat_gather_config(int bp, int wr, int R, int stages, bool onfly = false, bool exact = false,
-                                  bool weighted = false);   // 0 = choose automatically
+PatGatherConfig pat_gather_config(int bp, int wr, int R, int stages, bool onfly, bool exact, bool weighted,
+                                  const PatTune &env);      // 0 = choose automatically
 size_t pat_gather_smem_bytes(const PatGatherConfig &c);
 int pat_gather_occupancy(const PatGatherConfig &c, int *per_sm);
 int pat_launch_gather(const PatLaunchCtx &ctx, const PatGatherConfig &c, const float *u_t, const float *b,
@@ -169,7 +190,9 @@ int pat_launch_gather(const PatLaunchCtx &ctx, const PatGatherConfig &c, const f
                       unsigned long long *trace = nullptr,    // trace: per-CTA timeline, 8 x u64 per CTA, or NULL
                       const PatOnfly *onfly = nullptr,        // conventional BP: u computed in the kernel
                       float t0fs = 0.0f,                      // exact-time weightings: t0*fs
-                      const float *w_t = nullptr);            // pixel weights [ntiles][nsens][256] (cfg.weighted)
+                      const float *w_t = nullptr,             // pixel weights [ntiles][nsens][256] (cfg.weighted)
+                      uint32_t *ready = nullptr);             // counters of this call's b buffer: [0] pre-pass blocks done, [1] CTAs of
+                                                              // this grid done, [32] "b ready" flag (NULL: b is already there)
 
 // Set-up kernels of the pixel weights (weights.cu).
 int pat_launch_fill(const PatLaunchCtx &ctx, float *dst, int64_t n, float value);

@@ -9,6 +9,8 @@
 
 #include <cuda_runtime.h>
 
+#include <algorithm>
+
 namespace {
 
 // ---- table re-tiling: tau row-major [count][npix] -> u tile-major [tile][sensor][256] --------
@@ -85,6 +87,33 @@ __device__ __forceinline__ float4 weight_quad_interior(const float (&w)[6], int3
     return o;
 }
 
+// End of every pre-pass block (cross-call overlap, pat_api.cu "launch chain").  The gather of the same call does not
+// wait for this KERNEL to complete -- under a programmatic launch that would also wait for the previous call's
+// gather -- but for this counter to reach the number of blocks: each block publishes its stores (b and the zeroed
+// images) with a fence and adds 1.  Block 0 then waits for the grid's predecessor, so that the completion of this
+// kernel implies the completion of everything enqueued before it (a no-op without a programmatic edge).
+// ready[0] counts the blocks, ready[32] (its own 128-byte line: the gather's CTAs poll it, the atomics go elsewhere) is the
+// flag the last block raises.
+__device__ __forceinline__ unsigned long long pre_gtime() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ void prepass_block_done(uint32_t *ready, unsigned long long *trace = nullptr) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        if (ready) {
+            __threadfence();                                                   // release: this block's stores ...
+            const uint32_t n = gridDim.x * gridDim.y * gridDim.z;
+            if (atomicAdd(ready, 1u) == n - 1u) {
+                __threadfence();                                               // ... and, through the counter, everybody's
+                *reinterpret_cast<volatile uint32_t *>(ready + 32) = 1u;
+                if (trace) trace[1] = pre_gtime();
+            }
+        }
+    }
+}
+
 // Bp = 32 (interleaved layout [sensor][sample][32]).  Block = (128-sample chunk, sensor, frame group).
 // Phase 1: thread = (frame, 4 consecutive samples), a warp = 4 frames x 8 quads (four coalesced 128-byte
 // reads); H1 is applied right there and the four results go to shared memory out[sample][frame] with a
@@ -94,7 +123,7 @@ constexpr int kPreNs = 128;                                // samples per block
 __global__ void __launch_bounds__(256)
 prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
                int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int64_t npix, float wp, float wd,
-               float t0fs, int32_t n_lo) {
+               float t0fs, int32_t n_lo, uint32_t *ready) {
     asm volatile("griddepcontrol.launch_dependents;");
     __shared__ float out[kPreNs * 33];
     const int32_t s = blockIdx.y, grp = blockIdx.z, n_begin = n_lo + blockIdx.x * kPreNs;
@@ -149,6 +178,7 @@ prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *_
             dst[idx] = make_float4(t[0], t[1], t[2], t[3]);
         }
     }
+    prepass_block_done(ready);
 }
 
 // Bp = 4, 8: the BLOCKED layout b[g][sensor][n/32][frame][32] (gather.cu, PPL == 3).  One thread per
@@ -157,7 +187,7 @@ prepass_kernel(const float *__restrict__ traces, float *__restrict__ b, float *_
 __global__ void __launch_bounds__(256)
 prepass_blocked_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
                        int32_t nsens, int32_t nt, int32_t ntb, int32_t nframes, int32_t log2_bp,
-                       int64_t npix, float wp, float wd, float t0fs, int32_t n_lo, int32_t quads) {
+                       int64_t npix, float wp, float wd, float t0fs, int32_t n_lo, int32_t quads, uint32_t *ready) {
     asm volatile("griddepcontrol.launch_dependents;");
     // grid = (quads of the needed part of a row / 256, sensor, frame slot of the padded groups)
     const int32_t s = blockIdx.y, f = blockIdx.z, bp = 1 << log2_bp;
@@ -169,7 +199,7 @@ prepass_blocked_kernel(const float *__restrict__ traces, float *__restrict__ b, 
             for (int64_t q = blk * 256 + threadIdx.x; q < tot; q += nblk * 256) images[q] = 0.0f;
     }
     const int32_t q = blockIdx.x * 256 + threadIdx.x;
-    if (q >= quads) return;
+    if (q < quads) {
     const int32_t n0 = n_lo + (q << 2);
     float4 o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     if (f < nframes && quad_interior(n0, nt, wd)) {
@@ -187,13 +217,15 @@ prepass_blocked_kernel(const float *__restrict__ traces, float *__restrict__ b, 
     const int32_t g = f >> log2_bp, fl = f & (bp - 1);
     float *dst = b + (((((int64_t)g * nsens + s) * ntb + (n0 >> 5)) << log2_bp) + fl) * 32 + (n0 & 31);
     *reinterpret_cast<float4 *>(dst) = o;
+    }
+    prepass_block_done(ready);
 }
 
 // Bp = 16 (interleaved [sensor][sample][16], gather.cu PPL == 4).
 __global__ void __launch_bounds__(256)
 prepass_il16_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
                     int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int64_t npix, float wp, float wd,
-                    float t0fs, int32_t n_lo, int32_t quads) {
+                    float t0fs, int32_t n_lo, int32_t quads, uint32_t *ready) {
     asm volatile("griddepcontrol.launch_dependents;");
     {
         const int64_t nblk = (int64_t)gridDim.x * gridDim.y * gridDim.z;
@@ -206,7 +238,7 @@ prepass_il16_kernel(const float *__restrict__ traces, float *__restrict__ b, flo
     // contiguous bytes of each of 4 frame rows), four 16-byte stores (4 lanes = the 64-byte line of one sample)
     const int32_t s = blockIdx.y, grp = blockIdx.z, fq = (threadIdx.x & 3) << 2;
     const int32_t q = blockIdx.x * 64 + (threadIdx.x >> 2);
-    if (q >= quads) return;
+    if (q < quads) {
     const int32_t n0 = n_lo + (q << 2);
     float o[4][4];                                         // [sample][frame]
 #pragma unroll
@@ -238,48 +270,115 @@ prepass_il16_kernel(const float *__restrict__ traces, float *__restrict__ b, flo
 #pragma unroll
     for (int j = 0; j < 4; ++j)
         *reinterpret_cast<float4 *>(dst + j * 16) = make_float4(o[j][0], o[j][1], o[j][2], o[j][3]);
+    }
+    prepass_block_done(ready);
+}
+
+// Bp = 1, 16-byte aligned rows (nt % 4 == 0): the kernel of the bench headline, written to run BESIDE a running gather
+// (cross-call overlap, pat_api.cu).  There 3 gather CTAs leave 10240 registers per SM and every load queues behind
+// the gather's table stream (~2.5 us per round trip): the kernel must be ONE wave of small blocks that fit into that
+// remainder -- 128 threads x <= 64 registers -- whose threads take kB1U quads a quarter of the grid apart and issue
+// all their loads before they use any (a 256-thread block of 40 registers is an exact fit on paper and was not
+// co-scheduled: its blocks only started when gather CTAs left; one quad per thread needed two waves).
+constexpr int kB1Threads = 128, kB1U = 4;
+__global__ void __launch_bounds__(kB1Threads, 8)
+prepass_b1_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
+                  int32_t nsens, int32_t nt, int32_t nt4, int64_t npix, float wp, float wd, float t0fs,
+                  int32_t n_lo, int32_t quads, uint32_t *ready, unsigned long long *trace) {
+    asm volatile("griddepcontrol.launch_dependents;");
+    if (trace && blockIdx.x == 0 && threadIdx.x == 0) trace[0] = pre_gtime();
+    const uint32_t gid = blockIdx.x * kB1Threads + threadIdx.x, nthr = gridDim.x * kB1Threads;
+    for (uint32_t q = gid; q < (uint32_t)npix; q += nthr) images[q] = 0.0f;
+    const uint32_t total = (uint32_t)nsens * (uint32_t)quads;
+    for (uint32_t q = gid; q < total; q += kB1U * nthr) {
+        float w[kB1U][6];
+        uint32_t srow[kB1U];
+        int32_t n0[kB1U];
+#pragma unroll
+        for (int u = 0; u < kB1U; ++u) {
+            const uint32_t qq = min(q + u * nthr, total - 1u);                   // past the end: redo the last quad (harmless)
+            srow[u] = qq / (uint32_t)quads;
+            n0[u] = n_lo + (int32_t)((qq - srow[u] * (uint32_t)quads) << 2);
+            const float *p = traces + (size_t)srow[u] * nt + n0[u];
+            const float4 v = __ldg(reinterpret_cast<const float4 *>(p));
+            w[u][0] = n0[u] > 0 ? __ldg(p - 1) : 0.0f;
+            w[u][5] = n0[u] + 4 < nt ? __ldg(p + 4) : 0.0f;
+            w[u][1] = v.x; w[u][2] = v.y; w[u][3] = v.z; w[u][4] = v.w;
+        }
+#pragma unroll
+        for (int u = 0; u < kB1U; ++u) {
+            float4 o;
+            if (quad_interior(n0[u], nt, wd)) {
+                o = weight_quad_interior(w[u], n0[u], wp, t0fs);
+            } else {
+                o.x = weight_at(w[u] + 0, n0[u] + 0, nt, wp, wd, t0fs); o.y = weight_at(w[u] + 1, n0[u] + 1, nt, wp, wd, t0fs);
+                o.z = weight_at(w[u] + 2, n0[u] + 2, nt, wp, wd, t0fs); o.w = weight_at(w[u] + 3, n0[u] + 3, nt, wp, wd, t0fs);
+            }
+            *reinterpret_cast<float4 *>(b + (size_t)srow[u] * nt4 + n0[u]) = o;
+        }
+    }
+    prepass_block_done(ready, trace);
 }
 
 // Bp <= 2 (layout [sensor][sample][Bp]): one thread per 4 consecutive samples of all BP frames,
 // straight from global memory (the +-1 neighbours come from L1), BP 16-byte stores.
+constexpr int kSmallU = 1;                                 // quads per thread and loop iteration (generic Bp <= 2 kernel)
 template <int BP>
 __global__ void __launch_bounds__(256)
 prepass_small_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
                      int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int64_t npix, float wp, float wd,
-                     float t0fs, int32_t n_lo, int32_t quads) {
+                     float t0fs, int32_t n_lo, int32_t quads, uint32_t *ready, unsigned long long *trace) {
     asm volatile("griddepcontrol.launch_dependents;");
+    if (trace && blockIdx.x == 0 && threadIdx.x == 0) trace[0] = pre_gtime();
     const int64_t gid = (int64_t)blockIdx.x * 256 + threadIdx.x, nthr = (int64_t)gridDim.x * 256;
     for (int64_t q = gid; q < npix * nframes; q += nthr) images[q] = 0.0f;
-    for (int64_t q = gid; q < (int64_t)nsens * quads; q += nthr) {
-        const int32_t s = (int32_t)(q / quads), n0 = n_lo + ((int32_t)(q - (int64_t)s * quads) << 2);
-        float o[4][BP];
+    const int64_t total = (int64_t)nsens * quads;
+    for (int64_t q = gid; q < total; q += kSmallU * nthr) {
+        float w[kSmallU][BP][6];
+        int32_t sv[kSmallU], nv[kSmallU];
 #pragma unroll
-        for (int f = 0; f < BP; ++f) {
-            const float *p = traces + ((int64_t)f * nsens + s) * nt;
-            float w[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};    // p[n0-1 .. n0+4]
-            if (f < nframes) {
+        for (int u = 0; u < kSmallU; ++u) {
+            const int64_t qq = q + u * nthr;
+            const int32_t s = (int32_t)(qq / quads), n0 = n_lo + ((int32_t)(qq - (int64_t)s * quads) << 2);
+            sv[u] = qq < total ? s : -1;
+            nv[u] = n0;
+#pragma unroll
+            for (int f = 0; f < BP; ++f) {
+#pragma unroll
+                for (int j = 0; j < 6; ++j) w[u][f][j] = 0.0f;                  // p[n0-1 .. n0+4]
+                if (sv[u] < 0 || f >= nframes) continue;
+                const float *p = traces + ((int64_t)f * nsens + s) * nt;
                 if ((nt & 3) == 0) {                       // rows are 16-byte aligned: one vector load + 2 halo
                     const float4 v = __ldg(reinterpret_cast<const float4 *>(p + n0));
-                    w[1] = v.x; w[2] = v.y; w[3] = v.z; w[4] = v.w;
-                    if (n0 > 0) w[0] = __ldg(p + n0 - 1);
-                    if (n0 + 4 < nt) w[5] = __ldg(p + n0 + 4);
+                    w[u][f][1] = v.x; w[u][f][2] = v.y; w[u][f][3] = v.z; w[u][f][4] = v.w;
+                    if (n0 > 0) w[u][f][0] = __ldg(p + n0 - 1);
+                    if (n0 + 4 < nt) w[u][f][5] = __ldg(p + n0 + 4);
                 } else {
 #pragma unroll
                     for (int j = 0; j < 6; ++j) {
                         const int32_t n = n0 - 1 + j;
-                        if (n >= 0 && n < nt) w[j] = __ldg(p + n);
+                        if (n >= 0 && n < nt) w[u][f][j] = __ldg(p + n);
                     }
                 }
             }
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-                o[j][f] = (f < nframes && n0 + j < nt) ? weight_at(w + j, n0 + j, nt, wp, wd, t0fs) : 0.0f;
         }
-        float4 *dst = reinterpret_cast<float4 *>(b + ((int64_t)s * nt4 + n0) * BP);
-        const float *flat = &o[0][0];                      // [sample][frame] = the output order
 #pragma unroll
-        for (int v = 0; v < BP; ++v) dst[v] = make_float4(flat[4 * v], flat[4 * v + 1], flat[4 * v + 2], flat[4 * v + 3]);
+        for (int u = 0; u < kSmallU; ++u) {
+            if (sv[u] < 0) continue;
+            const int32_t n0 = nv[u];
+            float o[4][BP];
+#pragma unroll
+            for (int f = 0; f < BP; ++f)
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    o[j][f] = (f < nframes && n0 + j < nt) ? weight_at(w[u][f] + j, n0 + j, nt, wp, wd, t0fs) : 0.0f;
+            float4 *dst = reinterpret_cast<float4 *>(b + ((int64_t)sv[u] * nt4 + n0) * BP);
+            const float *flat = &o[0][0];                      // [sample][frame] = the output order
+#pragma unroll
+            for (int v = 0; v < BP; ++v) dst[v] = make_float4(flat[4 * v], flat[4 * v + 1], flat[4 * v + 2], flat[4 * v + 3]);
+        }
     }
+    prepass_block_done(ready, trace);
 }
 
 // ---- exact-time weightings (PAT_W_*_EXACT; Eq. 7 read literally) ------------------------
@@ -294,7 +393,7 @@ template <int LAYOUT>
 __global__ void __launch_bounds__(256)
 prepass_exact_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
                      int32_t nsens, int32_t nt, int32_t nt4, int32_t ntb, int32_t nframes, int32_t log2_bp,
-                     int64_t npix, float wp, float wd, int32_t n_lo, int32_t quads) {
+                     int64_t npix, float wp, float wd, int32_t n_lo, int32_t quads, uint32_t *ready) {
     asm volatile("griddepcontrol.launch_dependents;");
     {
         const int64_t nblk = (int64_t)gridDim.x * gridDim.y * gridDim.z;
@@ -311,7 +410,7 @@ prepass_exact_kernel(const float *__restrict__ traces, float *__restrict__ b, fl
         q = blockIdx.x * (256 >> lf) + (threadIdx.x >> lf);
     }
     else             { f = blockIdx.z; q = blockIdx.x * 256 + threadIdx.x; }
-    if (q >= quads) return;
+    if (q < quads) {
     const int32_t n0 = n_lo + (q << 2);
     float pv[4] = {0.0f, 0.0f, 0.0f, 0.0f}, dv[4] = {0.0f, 0.0f, 0.0f, 0.0f};
     if (f < nframes && n0 < nt) {
@@ -345,6 +444,8 @@ prepass_exact_kernel(const float *__restrict__ traces, float *__restrict__ b, fl
 #pragma unroll
         for (int j = 0; j < 4; ++j) *reinterpret_cast<float2 *>(dst + ((int64_t)j << log2_bp)) = make_float2(pv[j], dv[j]);
     }
+    }
+    prepass_block_done(ready);
 }
 
 // ---- measurement only: the same bytes as one step, as a plain stream ----------------------------
@@ -397,79 +498,82 @@ int pat_launch_retile(const PatLaunchCtx &ctx, const float *src, float *u_t, con
     return (int)cudaGetLastError();
 }
 
+// One launch path for every pre-pass kernel (an ordinary launch: fully ordered behind its dependencies).
+template <typename... KArgs, typename... Args>
+static int launch_pre(const PatLaunchCtx &ctx, void (*kern)(KArgs...), dim3 grid, int threads, Args... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid;
+    cfg.blockDim = dim3((unsigned)threads);
+    cfg.stream = (cudaStream_t)ctx.stream;
+    // Highest launch priority: in a chained capture (pat_api.cu) the pre-pass of call j becomes ready while the gather
+    // of call j-1 still has CTAs waiting for SM slots; at equal priority the work distributor keeps a later grid
+    // behind such a backlog, and the pre-pass -- whose small blocks fit beside the resident gather CTAs -- would only
+    // start once that gather is fully resident (measured: P_j started 0.9 us after the END of gather j-2).
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributePriority;
+    attr[0].val.priority = ctx.high_priority;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return (int)cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, float *images,
                        int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp,
-                       int64_t npix, float wp, float wd, float t0fs, bool exact, int32_t n_lo, int32_t n_hi) {
+                       int64_t npix, float wp, float wd, float t0fs, bool exact, int32_t n_lo, int32_t n_hi,
+                       uint32_t *ready) {
     // Only samples [n_lo, n_hi) of b can be read by a valid pixel (the caller's k-ranges; whole quads): the rest
     // of b is left as it is.  The blocked layout works in whole 32-sample blocks.
     const int32_t ntb = (nt + 31) / 32;
-    cudaStream_t st = (cudaStream_t)ctx.stream;
     if (n_hi > nt4) n_hi = nt4;
     if (n_lo < 0 || n_lo >= n_hi) { n_lo = 0; n_hi = 4; }           // nothing needed: still zero the images
     n_lo &= ~3;
     const bool blocked = pat_gather_blocked(bp);
     if (blocked) { n_lo &= ~31; n_hi = (n_hi + 31) & ~31; if (n_hi > ntb * 32) n_hi = ntb * 32; }
     const int32_t quads = (n_hi - n_lo + 3) >> 2;
+    int log2_bp = 0;
+    while ((1 << log2_bp) < bp) ++log2_bp;
     if (exact) {                                   // bp counts channels, two per frame
         if (bp < 2 || bp > 32) return (int)cudaErrorInvalidValue;
-        int log2_bp = 0;
-        while ((1 << log2_bp) < bp) ++log2_bp;
         const int32_t fpg = bp / 2, groups = (nframes + fpg - 1) / fpg;
-        if (bp == 2) {
-            dim3 grid((unsigned)((quads + 255) / 256), (unsigned)nsens, (unsigned)groups);
-            prepass_exact_kernel<0><<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd, n_lo, quads);
-        } else if (blocked) {
-            dim3 grid((unsigned)((quads + 255) / 256), (unsigned)nsens, (unsigned)(groups * fpg));
-            prepass_exact_kernel<1><<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd, n_lo, quads);
-        } else {
-            const int32_t qpb = 256 / fpg;                 // quads per block
-            dim3 grid((unsigned)((quads + qpb - 1) / qpb), (unsigned)nsens, (unsigned)groups);
-            prepass_exact_kernel<2><<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd, n_lo, quads);
-        }
-        return (int)cudaGetLastError();
+        if (bp == 2)
+            return launch_pre(ctx, prepass_exact_kernel<0>, dim3((unsigned)((quads + 255) / 256), (unsigned)nsens, (unsigned)groups), 256,
+                              traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd, n_lo, quads, ready);
+        if (blocked)
+            return launch_pre(ctx, prepass_exact_kernel<1>, dim3((unsigned)((quads + 255) / 256), (unsigned)nsens, (unsigned)(groups * fpg)), 256,
+                              traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd, n_lo, quads, ready);
+        const int32_t qpb = 256 / fpg;                     // quads per block
+        return launch_pre(ctx, prepass_exact_kernel<2>, dim3((unsigned)((quads + qpb - 1) / qpb), (unsigned)nsens, (unsigned)groups), 256,
+                          traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd, n_lo, quads, ready);
     }
     if (bp <= 2) {
         const int64_t work = (int64_t)nsens * quads;
-        int64_t blocks = (work + 255) / 256;
-        if (blocks > (int64_t)ctx.num_sms * 16) blocks = (int64_t)ctx.num_sms * 16;
+        int64_t blocks = (work + 256 * kSmallU - 1) / (256 * kSmallU);
+        if (blocks > (int64_t)ctx.num_sms * 8) blocks = (int64_t)ctx.num_sms * 8;
         if (blocks < 1) blocks = 1;
-        if (bp == 1 && ctx.xstep) {                 // measurement only: programmatic launch, no wait in the kernel
-            cudaLaunchConfig_t cfg{};
-            cfg.gridDim = dim3((unsigned)blocks);
-            cfg.blockDim = dim3(256);
-            cfg.stream = st;
-            cudaLaunchAttribute attr[1];
-            attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-            attr[0].val.programmaticStreamSerializationAllowed = 1;
-            cfg.attrs = attr;
-            cfg.numAttrs = 1;
-            return (int)cudaLaunchKernelEx(&cfg, prepass_small_kernel<1>, traces, b, images, nsens, nt, nt4, nframes, npix,
-                                           wp, wd, t0fs, n_lo, quads);
+        if (bp == 1 && (nt & 3) == 0 && nframes == 1 && work < (1ll << 31) && npix < (1ll << 32)) {
+            int64_t nb = (work + kB1Threads * kB1U - 1) / (kB1Threads * kB1U);   // one wave on configs[1] (130 blocks)
+            if (nb > (int64_t)ctx.num_sms * 8) nb = (int64_t)ctx.num_sms * 8;
+            return launch_pre(ctx, prepass_b1_kernel, dim3((unsigned)std::max<int64_t>(nb, 1)), kB1Threads, traces, b, images,
+                              nsens, nt, nt4, npix, wp, wd, t0fs, n_lo, quads, ready, ctx.pre_trace);
         }
         if (bp == 1)
-            prepass_small_kernel<1><<<(unsigned)blocks, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs, n_lo, quads);
-        else
-            prepass_small_kernel<2><<<(unsigned)blocks, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs, n_lo, quads);
-        return (int)cudaGetLastError();
+            return launch_pre(ctx, prepass_small_kernel<1>, dim3((unsigned)blocks), 256, traces, b, images, nsens, nt, nt4,
+                              nframes, npix, wp, wd, t0fs, n_lo, quads, ready, ctx.pre_trace);
+        return launch_pre(ctx, prepass_small_kernel<2>, dim3((unsigned)blocks), 256, traces, b, images, nsens, nt, nt4,
+                          nframes, npix, wp, wd, t0fs, n_lo, quads, ready, ctx.pre_trace);
     }
-    int log2_bp = 0;
-    while ((1 << log2_bp) < bp) ++log2_bp;
     if (blocked) {
         const int32_t groups = (nframes + bp - 1) / bp;
-        dim3 grid((unsigned)((quads + 255) / 256), (unsigned)nsens, (unsigned)(groups * bp));
-        prepass_blocked_kernel<<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, ntb, nframes, log2_bp, npix, wp, wd, t0fs,
-                                                     n_lo, quads);
-        return (int)cudaGetLastError();
+        return launch_pre(ctx, prepass_blocked_kernel, dim3((unsigned)((quads + 255) / 256), (unsigned)nsens, (unsigned)(groups * bp)), 256,
+                          traces, b, images, nsens, nt, ntb, nframes, log2_bp, npix, wp, wd, t0fs, n_lo, quads, ready);
     }
     if (bp == 16) {
         const int32_t groups = (nframes + 15) / 16;
-        dim3 grid((unsigned)((quads + 63) / 64), (unsigned)nsens, (unsigned)groups);
-        prepass_il16_kernel<<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs, n_lo, quads);
-        return (int)cudaGetLastError();
+        return launch_pre(ctx, prepass_il16_kernel, dim3((unsigned)((quads + 63) / 64), (unsigned)nsens, (unsigned)groups), 256,
+                          traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs, n_lo, quads, ready);
     }
     if (bp != 32) return (int)cudaErrorInvalidValue;
     const int32_t groups = (nframes + bp - 1) / bp;
-    dim3 grid((unsigned)((n_hi - n_lo + kPreNs - 1) / kPreNs), (unsigned)nsens, (unsigned)groups);
-    prepass_kernel<<<grid, 256, 0, st>>>(traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs, n_lo);
-    return (int)cudaGetLastError();
+    return launch_pre(ctx, prepass_kernel, dim3((unsigned)((n_hi - n_lo + kPreNs - 1) / kPreNs), (unsigned)nsens, (unsigned)groups), 256,
+                      traces, b, images, nsens, nt, nt4, nframes, npix, wp, wd, t0fs, n_lo, ready);
 }

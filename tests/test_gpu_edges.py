@@ -327,7 +327,6 @@ def test_back_to_back_single_frame_calls_on_one_plan():
     (the weighted-trace buffer and the images are reused by the next call's pre-pass: stream order must hold)."""
     import torch
     import paper_1501_03869_b200 as pat
-    mode = "default"
     geom, tau = case(1)
     rng = np.random.default_rng(77)
     plan = pat.Plan(geom.n, geom.h, geom.origin, None, geom.sensors, geom.roi_index, geom.nt, geom.fs, geom.t0, max_batch=1)
@@ -347,6 +346,6 @@ def test_back_to_back_single_frame_calls_on_one_plan():
         st.synchronize()
         for q in (0, 1, 5, 8, 9, 10, 11):
             ref = oracle.backproject(tau, trs[q].cpu().numpy(), geom.fs, geom.t0, 1)
-            assert_parity(outs[q].cpu().numpy(), ref, "back-to-back call %d, PAT_XSTEP=%s" % (q, mode))
+            assert_parity(outs[q].cpu().numpy(), ref, "back-to-back call %d" % q)
     finally:
         plan.close()
