@@ -386,6 +386,11 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
                          (double)nreal / (double)sc.nchunks, pat_gather_smem_bytes(cfg), per_sm);
         }
     }
+    const size_t main_entries = list.size();
+    try {                                                        // every CTA's first chunk once more, indexed by CTA
+        for (int64_t c = 0; c < G; ++c)
+            for (size_t q = 0; q < per_chunk; ++q) list.push_back(list[(size_t)cta_chunk[(size_t)c] * per_chunk + q]);
+    } catch (...) { return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
     cudaError_t ce = cudaMalloc(&sc.d_sched, list.size() * sizeof(Entry));
     if (ce == cudaSuccess) ce = cudaMalloc((void **)&sc.d_cta_chunk, cta_chunk.size() * sizeof(int32_t));
     if (ce == cudaSuccess) ce = cudaMemcpy(sc.d_sched, list.data(), list.size() * sizeof(Entry), cudaMemcpyHostToDevice);
@@ -396,6 +401,7 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
         if (sc.d_cta_chunk) cudaFree(sc.d_cta_chunk);
         return cuda_fail(p, ce, "work-list upload");
     }
+    sc.d_first = (char *)sc.d_sched + main_entries * sizeof(Entry);
     p->schedules.push_back(sc);
     *out = &p->schedules.back();
     return PAT_OK;
@@ -840,7 +846,7 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
         e = pat_launch_prepass(ctx, d_tr, bw, d_img, d.nsens, d.nt, p->nt4, nframes, bp, d.npix, p->wp, p->wd, t0fs, p->exact,
                                p->window_prepass ? (conventional ? p->onfly_lo : p->need_lo) : 0,
                                p->window_prepass ? (conventional ? p->onfly_hi : p->need_hi) : INT32_MAX,
-                               do_gather ? sync : nullptr);
+                               do_gather && !cp.chained ? sync : nullptr);   // chained: a full edge orders P before G
         if (e) return cuda_fail(p, e, "pre-pass launch");
         ++p->launches;
         if (cp.capture_id) capture_deps(st, &cid, &node_pre);
@@ -854,12 +860,12 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
             ctx.use_pdl = false;      // the edges are explicit: no launch attribute
             ++p->chained;
         }
-        e = pat_launch_gather(ctx, sc->cfg, (const float *)(p->ws + p->lay.tau), bw, sc->d_sched, sc->d_cta_chunk,
+        e = pat_launch_gather(ctx, sc->cfg, (const float *)(p->ws + p->lay.tau), bw, sc->d_sched, sc->d_first, sc->d_cta_chunk,
                               sc->grid_x, p->d_perm_masked ? p->d_perm_masked : (const int32_t *)(p->ws + p->lay.perm),
                               d_img, d.nsens, d.npix, d.nt,
                               p->nt4, nframes, p->trace_ctas == sc->grid_x ? p->trace_dev : nullptr,
                               conventional ? &onfly : nullptr, t0fs, p->d_w_t,
-                              do_pre ? sync : nullptr);
+                              do_pre && !cp.chained ? sync : nullptr);
         if (e) { p->sync_dirty = do_pre; return cuda_fail(p, e, "gather launch"); }
         ++p->launches;
         if (cp.capture_id) capture_deps(st, &cid, &node_gather);

@@ -80,7 +80,8 @@ struct PatSchedule {
     PatGatherConfig cfg;
     int grid_x = 0;
     int64_t nchunks = 0;
-    void *d_sched = nullptr;          // int4 [nchunks][R]
+    void *d_sched = nullptr;          // int4 [nchunks][R + 1], then [grid_x][R + 1]: every CTA's first chunk again
+    void *d_first = nullptr;          // = d_sched + nchunks*(R + 1) entries
     int32_t *d_cta_chunk = nullptr;   // int32 [grid_x + 1]
 };
 
@@ -185,7 +186,7 @@ PatGatherConfig pat_gather_config(int bp, int wr, int R, int stages, bool onfly,
 size_t pat_gather_smem_bytes(const PatGatherConfig &c);
 int pat_gather_occupancy(const PatGatherConfig &c, int *per_sm);
 int pat_launch_gather(const PatLaunchCtx &ctx, const PatGatherConfig &c, const float *u_t, const float *b,
-                      const void *sched, const int32_t *cta_chunk, int grid_x, const int32_t *perm,
+                      const void *sched, const void *first, const int32_t *cta_chunk, int grid_x, const int32_t *perm,
                       float *images, int32_t nsens, int64_t npix, int32_t nt, int32_t nt4, int32_t nframes,
                       unsigned long long *trace = nullptr,    // trace: per-CTA timeline, 8 x u64 per CTA, or NULL
                       const PatOnfly *onfly = nullptr,        // conventional BP: u computed in the kernel
