@@ -61,10 +61,44 @@ typedef struct {
     float   origin[3];          /* coordinates of node (0,0,0) [m] */
 } pat_grid;
 
+/* ---- device memory ---------------------------------------------------------------------------------------------
+ * The library never owns device memory it did not get from the caller.  Two channels:
+ *   1. the WORKSPACE of pat_plan_create: everything whose size follows from (nsens, npix, nt, max_batch) -- the
+ *      re-tiled table, the weighted traces (three buffers), staging for host-side inputs;
+ *   2. a PROVIDER installed with pat_set_device_allocator, for what depends on the data or on optional features:
+ *        - the work list of every frame-count class used (built at the first call of the class): per class about
+ *          16 bytes x (R + 1)/R per (tile, sensor) row that holds a valid pixel, R = rows per chunk (6 .. 24) -- 0.7 MB
+ *          for configs[1] (43 008 rows), ~0.6 GB for configs[4] (33.5 M rows);
+ *        - pat_set_pixel_weights / pat_compute_solid_angle_weights: a table of the size of the travel-time table;
+ *        - pat_backproject_conventional: 12 bytes per tile slot + 12 per sensor, and 8 bytes per (tile, sensor) row of
+ *          scratch while the row ranges of a new c0 are computed;
+ *        - pat_set_roi_mask: 4 bytes per tile slot;  pat_compute_solid_angle_weights: 24 bytes per tile slot of scratch;
+ *        - pat_eikonal_travel_times_device: one fp64 field per concurrently solved sensor (see there).
+ *      alloc(bytes, user) must return DEVICE memory, 256-byte aligned, valid until release(ptr, bytes, user), or NULL
+ *      (the call then fails with PAT_ERR_NOMEM).  Both are called on the calling thread, never from inside a stream
+ *      capture (nothing is allocated on the call path once a class's work list exists).  The provider is
+ *      process-wide; a plan keeps the one that was installed when it was created.  With no provider installed the
+ *      library's shim (csrc/alloc.cu) uses cudaMalloc / cudaFree.  pat_get_stats reports what a plan holds. */
+typedef void *(*pat_alloc_fn)(size_t bytes, void *user);
+typedef void (*pat_free_fn)(void *ptr, size_t bytes, void *user);
+pat_status pat_set_device_allocator(pat_alloc_fn alloc, pat_free_fn release, void *user);   /* both NULL: built-in shim */
+
+typedef struct {
+    int64_t workspace_bytes;        /* what pat_plan_workspace_bytes returned for this plan */
+    int64_t provider_bytes;         /* device memory currently held through the provider */
+    int64_t provider_bytes_peak;
+    int64_t work_list_bytes;        /* part of provider_bytes: the work lists built so far */
+    int64_t work_lists;             /* how many */
+    double  work_list_build_seconds;/* host time spent building them (first call of a frame-count class) */
+    int64_t kernel_launches, chained_calls;
+} pat_stats;
+pat_status pat_get_stats(const pat_plan *plan, pat_stats *out);
+
 /* Bytes of DEVICE workspace a plan with these sizes needs (0 on invalid sizes).
  * Layout: re-tiled table (the dominant term, 4*nsens*npix rounded up to whole
- * 256-pixel tiles), per-row sample ranges, weighted traces for max_batch frames (rounded up to
- * the frame-count class), staging for host-side inputs, pixel permutation. */
+ * 256-pixel tiles), per-row sample ranges, THREE buffers of weighted traces for max_batch frames (rounded up to
+ * the frame-count class; consecutive calls rotate through them, see pat_backproject), staging for host-side
+ * inputs, pixel permutation, counters. */
 size_t pat_plan_workspace_bytes(const pat_grid *grid, int32_t nsens, int64_t npix,
                                 int32_t nt, int32_t max_batch);
 

@@ -8,7 +8,8 @@ from .binding import (PAT_OK, PAT_ERR_INVALID_ARG, PAT_ERR_BAD_STATE, PAT_ERR_CU
                       PAT_ERR_UNSUPPORTED, PAT_W_DELAY_SUM, PAT_W_PAPER, PAT_W_PAPER_EXACT, PAT_W_UBP, PAT_W_UBP_EXACT, PatError, PatGrid,
                       lib, library_path, pat_plan_workspace_bytes, pat_plan_create,
                       pat_set_travel_times, pat_backproject, pat_destroy, pat_last_error,
-                      pat_kernel_launches, pat_chained_calls, pat_set_gather_tuning, pat_fmm_travel_times,
+                      pat_kernel_launches, pat_chained_calls, pat_set_device_allocator, pat_get_stats, install_torch_allocator,
+                      torch_alloc, torch_free, PatStats, pat_set_gather_tuning, pat_fmm_travel_times,
                       pat_compute_travel_times, pat_set_profiling, pat_get_profile,
                       pat_eikonal_travel_times_device, pat_compute_travel_times_gpu,
                       pat_backproject_conventional, pat_set_roi_mask, pat_set_pixel_weights,

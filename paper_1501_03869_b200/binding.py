@@ -39,6 +39,13 @@ class PatGrid(ctypes.Structure):
         return g
 
 
+class PatStats(ctypes.Structure):
+    _fields_ = [("workspace_bytes", ctypes.c_int64), ("provider_bytes", ctypes.c_int64),
+                ("provider_bytes_peak", ctypes.c_int64), ("work_list_bytes", ctypes.c_int64),
+                ("work_lists", ctypes.c_int64), ("work_list_build_seconds", ctypes.c_double),
+                ("kernel_launches", ctypes.c_int64), ("chained_calls", ctypes.c_int64)]
+
+
 def library_path():
     return os.path.join(_HERE, _LIBNAME)
 
@@ -73,6 +80,10 @@ def lib():
     L.pat_last_error.argtypes = [vp]
     L.pat_kernel_launches.restype = i64
     L.pat_kernel_launches.argtypes = [vp]
+    L.pat_set_device_allocator.restype = ctypes.c_int
+    L.pat_set_device_allocator.argtypes = [vp, vp, vp]
+    L.pat_get_stats.restype = ctypes.c_int
+    L.pat_get_stats.argtypes = [vp, ctypes.POINTER(PatStats)]
     L.pat_chained_calls.restype = i64
     L.pat_chained_calls.argtypes = [vp]
     L.pat_set_gather_tuning.restype = ctypes.c_int
@@ -103,6 +114,63 @@ def lib():
     L.pat_compute_travel_times_gpu.argtypes = [vp, i32, ctypes.POINTER(i32), vp]
     _lib = L
     return L
+
+
+# ---- device-memory provider (include/pat.h "device memory"): torch tensors, so that the caller's allocator owns
+# everything -- the library itself never calls cudaMalloc once a provider is installed -----------------------
+_ALLOC_CB = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
+_FREE_CB = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
+_provider = {"alloc": None, "free": None, "live": {}, "py_alloc": None, "py_free": None}
+
+
+def pat_set_device_allocator(alloc=None, free=None):
+    """alloc(nbytes) -> 256-byte aligned device address (int) or None; free(address, nbytes).  Both None: the
+    library's cudaMalloc shim again.  The callbacks are kept alive by this module."""
+    if (alloc is None) != (free is None):
+        raise ValueError("alloc and free must be given together")
+    if alloc is None:
+        st = lib().pat_set_device_allocator(None, None, None)
+        _provider.update(alloc=None, free=None, py_alloc=None, py_free=None)
+    else:
+        def _a(nbytes, _user):
+            try:
+                return alloc(int(nbytes))
+            except Exception:
+                return None
+        def _f(ptr, nbytes, _user):
+            try:
+                free(int(ptr), int(nbytes))
+            except Exception:
+                pass
+        ca, cf = _ALLOC_CB(_a), _FREE_CB(_f)
+        st = lib().pat_set_device_allocator(ctypes.cast(ca, ctypes.c_void_p), ctypes.cast(cf, ctypes.c_void_p), None)
+        _provider.update(alloc=ca, free=cf, py_alloc=alloc, py_free=free)
+    if st != PAT_OK:
+        raise PatError(st, "pat_set_device_allocator")
+
+
+def torch_alloc(nbytes):
+    import torch
+    t = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
+    ptr = (t.data_ptr() + 255) // 256 * 256
+    _provider["live"][ptr] = t
+    return ptr
+
+
+def torch_free(ptr, nbytes):
+    _provider["live"].pop(ptr, None)
+
+
+def install_torch_allocator():
+    """Make torch the provider (idempotent; does not replace a provider the caller has installed)."""
+    if _provider["alloc"] is None:
+        pat_set_device_allocator(torch_alloc, torch_free)
+
+
+def pat_get_stats(plan):
+    st = PatStats()
+    _check(plan, lib().pat_get_stats(plan, ctypes.byref(st)))
+    return {k: getattr(st, k) for k, _ in PatStats._fields_}
 
 
 def _addr(a):
@@ -250,6 +318,7 @@ def pat_eikonal_travel_times_device(grid, c_map, sensor_xyz, nsens, roi_index, n
                                     tau_out, max_rounds=0, stream=None):
     """GPU fast-sweeping solve (include/pat.h); tau_out is a DEVICE fp32 [count][npix] tensor.
     Returns the largest number of rounds any sensor needed."""
+    install_torch_allocator()
     r = ctypes.c_int32()
     st = lib().pat_eikonal_travel_times_device(ctypes.byref(grid), _addr(c_map), _addr(sensor_xyz), nsens,
                                                _addr(roi_index) if roi_index is not None else None, npix,
@@ -272,6 +341,7 @@ class Plan:
     def __init__(self, n, h, origin, c_map, sensor_xyz, roi_index, nt, fs, t0=0.0,
                  weighting=PAT_W_PAPER, max_batch=1, device="cuda", nsens=None):
         import torch
+        install_torch_allocator()
         self.grid = PatGrid.make(n, h, origin)
         self.c_map = None if c_map is None else np.ascontiguousarray(c_map, dtype=np.float32).ravel()
         self.sensor_xyz = None if sensor_xyz is None else np.ascontiguousarray(sensor_xyz, dtype=np.float32)
@@ -325,6 +395,9 @@ class Plan:
 
     def chained_calls(self):
         return pat_chained_calls(self.handle)
+
+    def stats(self):
+        return pat_get_stats(self.handle)
 
     def close(self):
         if getattr(self, "handle", None):

@@ -217,25 +217,28 @@ extern "C" pat_status pat_eikonal_travel_times_device(const pat_grid *grid, cons
     if (const char *ev = std::getenv("PAT_EIK_SLOTS")) slots = std::max<int64_t>(1, std::min<int64_t>(slots, std::atoi(ev)));
 
     cudaStream_t st = (cudaStream_t)stream;
-    double *d_sh = nullptr, *d_T = nullptr, *d_sv = nullptr;
-    int32_t *d_sn = nullptr, *d_info = nullptr;
-    int64_t *d_roi = nullptr;
-    auto cleanup = [&]() {
-        cudaFree(d_sh); cudaFree(d_T); cudaFree(d_sv); cudaFree(d_sn); cudaFree(d_info); cudaFree(d_roi);
-    };
-    cudaError_t e = cudaMalloc((void **)&d_sh, (size_t)P.N * 8);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&d_T, (size_t)slots * P.N * 8);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&d_sv, seed_val.size() * 8);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&d_sn, seed_node.size() * 4);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&d_info, 8);
-    if (e == cudaSuccess && roi_index) e = cudaMalloc((void **)&d_roi, (size_t)npix * 8);
+    // scratch: one block from the caller's device-memory provider (alloc.cu), carved into
+    // [slowness*h][T fields of the concurrent sensors][seed values][seed nodes][info][roi indices]
+    const PatAllocator alloc = pat_current_allocator();
+    auto up = [](size_t v) { return (v + 255) / 256 * 256; };
+    const size_t o_sh = 0, o_T = o_sh + up((size_t)P.N * 8), o_sv = o_T + up((size_t)slots * P.N * 8),
+                 o_sn = o_sv + up(seed_val.size() * 8), o_info = o_sn + up(seed_node.size() * 4), o_roi = o_info + 256,
+                 total_bytes = o_roi + (roi_index ? up((size_t)npix * 8) : 0);
+    PatDevBuf buf;
+    if (!pat_dev_alloc(alloc, total_bytes, &buf)) return PAT_ERR_NOMEM;
+    char *base = (char *)buf.p;
+    double *d_sh = (double *)(base + o_sh), *d_T = (double *)(base + o_T), *d_sv = (double *)(base + o_sv);
+    int32_t *d_sn = (int32_t *)(base + o_sn), *d_info = (int32_t *)(base + o_info);
+    int64_t *d_roi = roi_index ? (int64_t *)(base + o_roi) : nullptr;
+    auto cleanup = [&]() { pat_dev_free(alloc, &buf); };
+    cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_sh, sh.data(), (size_t)P.N * 8, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_sv, seed_val.data(), seed_val.size() * 8, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_sn, seed_node.data(), seed_node.size() * 4, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess && roi_index)
         e = cudaMemcpyAsync(d_roi, roi_index, (size_t)npix * 8, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(d_info, 0, 8, st);
-    if (e != cudaSuccess) { cleanup(); return e == cudaErrorMemoryAllocation ? PAT_ERR_NOMEM : PAT_ERR_CUDA; }
+    if (e != cudaSuccess) { cudaStreamSynchronize(st); cleanup(); return PAT_ERR_CUDA; }
     P.sh = d_sh; P.T = d_T; P.seed_val = d_sv; P.seed_node = d_sn; P.roi = d_roi; P.npix = npix;
     P.tau_out = tau_out; P.count = count; P.max_rounds = max_rounds; P.info = d_info;
     if (nd == 2) eikonal_sweep_kernel<2><<<(unsigned)slots, threads, 0, st>>>(P);

@@ -6,6 +6,7 @@
 
 #include <algorithm>
 #include <atomic>
+#include <chrono>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -206,11 +207,14 @@ void needed_samples(const std::vector<int32_t> &meta, int32_t nt, int32_t *lo, i
     *hi = std::min(nt, (kmax + 3 + 3) & ~3);
 }
 
+// Device memory of the plan beyond its workspace: from the caller's provider (alloc.cu), accounted per plan.
+bool plan_alloc(pat_plan *p, size_t bytes, PatDevBuf *out) {
+    return pat_dev_alloc(p->alloc, bytes, out, &p->dev_bytes, &p->dev_bytes_peak);
+}
+void plan_free(pat_plan *p, PatDevBuf *buf) { pat_dev_free(p->alloc, buf, &p->dev_bytes); }
+
 void drop_schedules(pat_plan *p) {
-    for (PatSchedule &sc : p->schedules) {
-        if (sc.d_sched) cudaFree(sc.d_sched);
-        if (sc.d_cta_chunk) cudaFree(sc.d_cta_chunk);
-    }
+    for (PatSchedule &sc : p->schedules) plan_free(p, &sc.buf);
     p->schedules.clear();
 }
 
@@ -391,17 +395,20 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
         for (int64_t c = 0; c < G; ++c)
             for (size_t q = 0; q < per_chunk; ++q) list.push_back(list[(size_t)cta_chunk[(size_t)c] * per_chunk + q]);
     } catch (...) { return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
-    cudaError_t ce = cudaMalloc(&sc.d_sched, list.size() * sizeof(Entry));
-    if (ce == cudaSuccess) ce = cudaMalloc((void **)&sc.d_cta_chunk, cta_chunk.size() * sizeof(int32_t));
-    if (ce == cudaSuccess) ce = cudaMemcpy(sc.d_sched, list.data(), list.size() * sizeof(Entry), cudaMemcpyHostToDevice);
+    // one block from the caller's provider: [chunk entries][first-chunk copies][CTA ranges]
+    const size_t list_bytes = list.size() * sizeof(Entry);
+    if (!plan_alloc(p, list_bytes + cta_chunk.size() * sizeof(int32_t), &sc.buf))
+        return fail(p, PAT_ERR_NOMEM, "work list: the device-memory provider returned nothing");
+    sc.d_sched = sc.buf.p;
+    sc.d_first = (char *)sc.buf.p + main_entries * sizeof(Entry);
+    sc.d_cta_chunk = (int32_t *)((char *)sc.buf.p + list_bytes);
+    cudaError_t ce = cudaMemcpy(sc.d_sched, list.data(), list_bytes, cudaMemcpyHostToDevice);
     if (ce == cudaSuccess)
         ce = cudaMemcpy(sc.d_cta_chunk, cta_chunk.data(), cta_chunk.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
     if (ce != cudaSuccess) {
-        if (sc.d_sched) cudaFree(sc.d_sched);
-        if (sc.d_cta_chunk) cudaFree(sc.d_cta_chunk);
+        plan_free(p, &sc.buf);
         return cuda_fail(p, ce, "work-list upload");
     }
-    sc.d_first = (char *)sc.d_sched + main_entries * sizeof(Entry);
     p->schedules.push_back(sc);
     *out = &p->schedules.back();
     return PAT_OK;
@@ -410,6 +417,11 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
 pat_status get_schedule(pat_plan *p, int bp, bool onfly, PatSchedule **out) {
     for (PatSchedule &sc : p->schedules)
         if (sc.cfg.bp == bp && sc.cfg.onfly == onfly) { *out = &sc; return PAT_OK; }
+    const auto t_begin = std::chrono::steady_clock::now();
+    struct Timer {
+        pat_plan *p; std::chrono::steady_clock::time_point t0;
+        ~Timer() { p->sched_build_seconds += std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count(); ++p->sched_builds; }
+    } timer{p, t_begin};
     PatGatherConfig cfg = pat_gather_config(bp, p->tune_wr, p->tune_R, p->tune_stages, onfly, p->exact,
                                             p->d_w_t != nullptr, p->env);
     return build_schedule(p, cfg, out);
@@ -436,12 +448,15 @@ pat_status ensure_onfly(pat_plan *p, float c0, void *stream, PatOnfly *out) {
                 pix[(size_t)dd * slots + sl] = dd < p->grid.ndim ? p->grid.origin[dd] + stepv : 0.0f;
             }
         }
-        cudaError_t e = cudaMalloc((void **)&p->d_pix, pix.size() * sizeof(float));
-        if (e == cudaSuccess) e = cudaMalloc((void **)&p->d_sens, (size_t)S * 3 * sizeof(float));
-        if (e == cudaSuccess) e = cudaMemcpy(p->d_pix, pix.data(), pix.size() * sizeof(float), cudaMemcpyHostToDevice);
+        const size_t pix_bytes = align_up(pix.size() * sizeof(float), 256);
+        if (!plan_alloc(p, pix_bytes + (size_t)S * 3 * sizeof(float), &p->onfly_buf))
+            return fail(p, PAT_ERR_NOMEM, "conventional BP geometry: the device-memory provider returned nothing");
+        p->d_pix = (float *)p->onfly_buf.p;
+        p->d_sens = (float *)((char *)p->onfly_buf.p + pix_bytes);
+        cudaError_t e = cudaMemcpy(p->d_pix, pix.data(), pix.size() * sizeof(float), cudaMemcpyHostToDevice);
         if (e == cudaSuccess) e = cudaMemcpy(p->d_sens, p->sensors.data(), (size_t)S * 3 * sizeof(float), cudaMemcpyHostToDevice);
         if (e != cudaSuccess) {
-            cudaFree(p->d_pix); cudaFree(p->d_sens);
+            plan_free(p, &p->onfly_buf);
             p->d_pix = p->d_sens = nullptr;
             return cuda_fail(p, e, "conventional BP geometry upload");
         }
@@ -450,24 +465,26 @@ pat_status ensure_onfly(pat_plan *p, float c0, void *stream, PatOnfly *out) {
     out->inv_c0 = 1.0f / c0; out->t0 = p->t0; out->fs = p->fs; out->ndim = p->grid.ndim;
     if (p->onfly_c0 != c0 || p->onfly_meta.empty()) {
         const int64_t nrows = p->dims.ntiles * S;
-        void *d_meta = nullptr;
-        cudaError_t e = cudaMalloc(&d_meta, (size_t)nrows * 8);
-        if (e != cudaSuccess) return cuda_fail(p, e, "conventional BP row ranges");
+        // scratch for the row ranges: the workspace's meta array is the table path's; same size, own block
+        PatDevBuf mbuf;
+        if (!plan_alloc(p, (size_t)nrows * 8, &mbuf))
+            return fail(p, PAT_ERR_NOMEM, "conventional BP row ranges: the device-memory provider returned nothing");
+        void *d_meta = mbuf.p;
+        cudaError_t e = cudaSuccess;
         PatLaunchCtx ctx{stream, p->num_sms, false};
         int le = pat_launch_onfly_meta(ctx, *out, S, d_meta, nrows, p->dims.nt);
         ++p->launches;
-        try { p->onfly_meta.resize((size_t)nrows * 2); } catch (...) { cudaFree(d_meta); return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
+        try { p->onfly_meta.resize((size_t)nrows * 2); } catch (...) { cudaStreamSynchronize(st); plan_free(p, &mbuf); return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
         if (!le) e = cudaMemcpyAsync(p->onfly_meta.data(), d_meta, (size_t)nrows * 8, cudaMemcpyDeviceToHost, st);
         if (!le && e == cudaSuccess) e = cudaStreamSynchronize(st);
-        cudaFree(d_meta);
+        plan_free(p, &mbuf);
         if (le || e != cudaSuccess) { p->onfly_meta.clear(); return cuda_fail(p, le ? le : (int)e, "conventional BP row ranges"); }
         p->onfly_c0 = c0;
         needed_samples(p->onfly_meta, p->dims.nt, &p->onfly_lo, &p->onfly_hi);
         // work lists of the previous c0 are stale
         for (size_t q = 0; q < p->schedules.size();) {
             if (p->schedules[q].cfg.onfly) {
-                if (p->schedules[q].d_sched) cudaFree(p->schedules[q].d_sched);
-                if (p->schedules[q].d_cta_chunk) cudaFree(p->schedules[q].d_cta_chunk);
+                plan_free(p, &p->schedules[q].buf);
                 p->schedules.erase(p->schedules.begin() + (long)q);
             } else {
                 ++q;
@@ -628,6 +645,7 @@ extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, cons
     }
     p->device = dev;
     p->num_sms = sms;
+    p->alloc = pat_current_allocator();
     {
         int lo = 0, hi = 0;
         if (cudaDeviceGetStreamPriorityRange(&lo, &hi) == cudaSuccess) p->prio_high = hi; else cudaGetLastError();
@@ -828,7 +846,8 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
         return PAT_OK;
     }
     if (do_gather && p->trace_file && !p->trace_dev && nframes <= 32) {   // diagnostic timeline (PAT_TRACE_FILE at create)
-        if (cudaMalloc((void **)&p->trace_dev, (size_t)(sc->grid_x + 1) * 8 * sizeof(unsigned long long)) == cudaSuccess) {
+        if (plan_alloc(p, (size_t)(sc->grid_x + 1) * 8 * sizeof(unsigned long long), &p->trace_buf)) {
+            p->trace_dev = (unsigned long long *)p->trace_buf.p;
             p->trace_ctas = sc->grid_x;
             cudaMemset(p->trace_dev, 0, (size_t)(sc->grid_x + 1) * 8 * sizeof(unsigned long long));
         } else {
@@ -895,14 +914,13 @@ extern "C" pat_status pat_destroy(pat_plan *p) {
                 const std::string fn = p->trace_file_name + "." + std::to_string(serial.fetch_add(1));
                 if (FILE *f = std::fopen(fn.c_str(), "wb")) { std::fwrite(h.data(), 8, h.size(), f); std::fclose(f); }
             }
-        cudaFree(p->trace_dev);
+        plan_free(p, &p->trace_buf);
     }
     if (p) {
         drop_events(p); drop_schedules(p);
-        if (p->d_perm_masked) cudaFree(p->d_perm_masked);
-        if (p->d_w_t) cudaFree(p->d_w_t);
-        if (p->d_pix) cudaFree(p->d_pix);
-        if (p->d_sens) cudaFree(p->d_sens);
+        plan_free(p, &p->mask_buf);
+        plan_free(p, &p->w_buf);
+        plan_free(p, &p->onfly_buf);
         if (p->copy_stream) { cudaStreamSynchronize((cudaStream_t)p->copy_stream); cudaStreamDestroy((cudaStream_t)p->copy_stream); }
         for (int q = 0; q < 2; ++q) {
             if (p->ev_h2d[q]) cudaEventDestroy((cudaEvent_t)p->ev_h2d[q]);
@@ -950,6 +968,20 @@ extern "C" const char *pat_last_error(const pat_plan *p) {
 extern "C" int64_t pat_kernel_launches(const pat_plan *p) { return p ? p->launches : 0; }
 
 extern "C" int64_t pat_chained_calls(const pat_plan *p) { return p ? p->chained : 0; }
+
+extern "C" pat_status pat_get_stats(const pat_plan *p, pat_stats *out) {
+    if (!p || !out) return PAT_ERR_INVALID_ARG;
+    std::memset(out, 0, sizeof(*out));
+    out->workspace_bytes = (int64_t)p->lay.total;
+    out->provider_bytes = p->dev_bytes;
+    out->provider_bytes_peak = p->dev_bytes_peak;
+    for (const PatSchedule &sc : p->schedules) out->work_list_bytes += (int64_t)sc.buf.bytes;
+    out->work_lists = p->sched_builds;
+    out->work_list_build_seconds = p->sched_build_seconds;
+    out->kernel_launches = p->launches;
+    out->chained_calls = p->chained;
+    return PAT_OK;
+}
 
 extern "C" pat_status pat_get_trace_window(const pat_plan *p, int32_t *first, int32_t *count) {
     if (!p || !first || !count) return PAT_ERR_INVALID_ARG;
@@ -1023,11 +1055,12 @@ static pat_status ensure_weight_table(pat_plan *p, void *stream) {
     cudaError_t e = cudaDeviceSynchronize();            // no launch may still use the unweighted work lists
     if (e != cudaSuccess) return cuda_fail(p, e, "synchronise");
     const int64_t n = p->dims.ntiles * (int64_t)p->dims.nsens * kTilePix;
-    e = cudaMalloc((void **)&p->d_w_t, (size_t)n * sizeof(float));
-    if (e != cudaSuccess) { p->d_w_t = nullptr; return cuda_fail(p, e, "weight table allocation"); }
+    if (!plan_alloc(p, (size_t)n * sizeof(float), &p->w_buf))
+        return fail(p, PAT_ERR_NOMEM, "weight table: the device-memory provider returned nothing");
+    p->d_w_t = (float *)p->w_buf.p;
     PatLaunchCtx ctx{stream, p->num_sms, false};
     int le = pat_launch_fill(ctx, p->d_w_t, n, 1.0f);
-    if (le) { cudaFree(p->d_w_t); p->d_w_t = nullptr; return cuda_fail(p, le, "weight table fill"); }
+    if (le) { plan_free(p, &p->w_buf); p->d_w_t = nullptr; return cuda_fail(p, le, "weight table fill"); }
     ++p->launches;
     drop_schedules(p);                                  // the stages now hold weight rows as well
     return PAT_OK;
@@ -1041,7 +1074,7 @@ extern "C" pat_status pat_set_pixel_weights(pat_plan *p, const float *w, int32_t
         if (p->d_w_t) {
             cudaError_t e = cudaDeviceSynchronize();
             if (e != cudaSuccess) return cuda_fail(p, e, "synchronise");
-            cudaFree(p->d_w_t);
+            plan_free(p, &p->w_buf);
             p->d_w_t = nullptr;
             drop_schedules(p);
         }
@@ -1076,11 +1109,14 @@ extern "C" pat_status pat_compute_solid_angle_weights(pat_plan *p, const float *
         for (int dd = 0; dd < p->grid.ndim; ++dd)
             pix[(size_t)dd * slots + sl] = (double)p->grid.origin[dd] + (double)id[dd] * (double)p->grid.h;
     }
-    double *d_pix = nullptr;
-    float *d_sn = nullptr;                              // sensors, then normals
     cudaStream_t cs = (cudaStream_t)stream;
-    cudaError_t e = cudaMalloc((void **)&d_pix, pix.size() * sizeof(double));
-    if (e == cudaSuccess) e = cudaMalloc((void **)&d_sn, (size_t)S * 6 * sizeof(float));
+    PatDevBuf tmp;                                      // node coordinates, then sensors, then normals
+    const size_t pix_bytes = align_up(pix.size() * sizeof(double), 256);
+    if (!plan_alloc(p, pix_bytes + (size_t)S * 6 * sizeof(float), &tmp))
+        return fail(p, PAT_ERR_NOMEM, "solid-angle scratch: the device-memory provider returned nothing");
+    double *d_pix = (double *)tmp.p;
+    float *d_sn = (float *)((char *)tmp.p + pix_bytes);
+    cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_pix, pix.data(), pix.size() * sizeof(double), cudaMemcpyHostToDevice, cs);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_sn, p->sensors.data(), (size_t)S * 3 * sizeof(float), cudaMemcpyHostToDevice, cs);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_sn + (size_t)S * 3, normals, (size_t)S * 3 * sizeof(float), cudaMemcpyHostToDevice, cs);
@@ -1091,8 +1127,8 @@ extern "C" pat_status pat_compute_solid_angle_weights(pat_plan *p, const float *
         ++p->launches;
     }
     if (e == cudaSuccess && !le) e = cudaStreamSynchronize(cs);       // the host arrays are only borrowed
-    cudaFree(d_pix);
-    cudaFree(d_sn);
+    else cudaStreamSynchronize(cs);
+    plan_free(p, &tmp);
     if (le) return cuda_fail(p, le, "solid-angle launch");
     if (e != cudaSuccess) return cuda_fail(p, e, "solid-angle weights");
     return PAT_OK;
@@ -1105,7 +1141,8 @@ extern "C" pat_status pat_set_roi_mask(pat_plan *p, const uint8_t *mask) {
     drop_schedules(p);
     if (!mask) {
         p->tile_active.clear();
-        if (p->d_perm_masked) { cudaFree(p->d_perm_masked); p->d_perm_masked = nullptr; }
+        plan_free(p, &p->mask_buf);
+        p->d_perm_masked = nullptr;
         return PAT_OK;
     }
     const int64_t slots = p->dims.ntiles * kTilePix;
@@ -1121,8 +1158,11 @@ extern "C" pat_status pat_set_roi_mask(pat_plan *p, const uint8_t *mask) {
         else perm[(size_t)sl] = -1;
     }
     if (!p->d_perm_masked) {
-        e = cudaMalloc((void **)&p->d_perm_masked, (size_t)slots * sizeof(int32_t));
-        if (e != cudaSuccess) { p->d_perm_masked = nullptr; p->tile_active.clear(); return cuda_fail(p, e, "roi mask allocation"); }
+        if (!plan_alloc(p, (size_t)slots * sizeof(int32_t), &p->mask_buf)) {
+            p->tile_active.clear();
+            return fail(p, PAT_ERR_NOMEM, "roi mask: the device-memory provider returned nothing");
+        }
+        p->d_perm_masked = (int32_t *)p->mask_buf.p;
     }
     e = cudaMemcpy(p->d_perm_masked, perm.data(), (size_t)slots * sizeof(int32_t), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) return cuda_fail(p, e, "roi mask upload");

@@ -75,13 +75,21 @@ struct PatOnfly {
     int32_t ndim = 2;
 };
 
-// Host-built work list of one PatGatherConfig (built lazily, library-owned device memory).
+// Device memory the library asks for on its own goes through the caller's provider (alloc.cu).
+struct PatAllocator { pat_alloc_fn alloc = nullptr; pat_free_fn release = nullptr; void *user = nullptr; };
+struct PatDevBuf { void *p = nullptr; size_t bytes = 0; };
+PatAllocator pat_current_allocator();
+bool pat_dev_alloc(const PatAllocator &a, size_t bytes, PatDevBuf *out, int64_t *held = nullptr, int64_t *peak = nullptr);
+void pat_dev_free(const PatAllocator &a, PatDevBuf *buf, int64_t *held = nullptr);
+
+// Host-built work list of one PatGatherConfig (built lazily; device memory from the caller's provider).
 struct PatSchedule {
     PatGatherConfig cfg;
     int grid_x = 0;
     int64_t nchunks = 0;
-    void *d_sched = nullptr;          // int4 [nchunks][R + 1], then [grid_x][R + 1]: every CTA's first chunk again
-    void *d_first = nullptr;          // = d_sched + nchunks*(R + 1) entries
+    PatDevBuf buf;                    // one block: the three arrays below
+    void *d_sched = nullptr;          // int4 [nchunks][R + 1]
+    void *d_first = nullptr;          // int4 [grid_x][R + 1]: every CTA's first chunk again, indexed by CTA
     int32_t *d_cta_chunk = nullptr;   // int32 [grid_x + 1]
 };
 
@@ -118,6 +126,11 @@ struct pat_plan {
     int64_t chained = 0;              // calls whose pre-pass was launched with a programmatic edge (launch chain)
     bool trace_file = false;                   // PAT_TRACE_FILE was set at create
     std::string trace_file_name;
+    PatAllocator alloc;                        // the device-memory provider as it was at pat_plan_create
+    int64_t dev_bytes = 0, dev_bytes_peak = 0; // device memory currently / at most held through it
+    int64_t sched_builds = 0;                  // work lists built so far, and the host seconds that took
+    double sched_build_seconds = 0.0;
+    PatDevBuf trace_buf, onfly_buf, w_buf, mask_buf;
     unsigned long long *trace_dev = nullptr;   // PAT_TRACE_FILE diagnostic: timeline of the last gather launch
     int trace_ctas = 0;
     // host-buffer calls: H2D on an own copy stream into alternating staging buffers, so that the transfer

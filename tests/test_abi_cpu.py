@@ -159,3 +159,13 @@ def test_workload_roi_counts_match_the_paper():
     g = W.make_geometry(1)
     assert g.npix == int(want["npix_coarse"]) and g.nsens == int(want["nsens"])
     assert np.all(np.diff(g.roi_index) > 0)
+
+
+def test_device_allocator_abi_without_a_gpu():
+    """pat_set_device_allocator: both callbacks or none (argument check only; nothing is allocated here)."""
+    import ctypes
+    L = pat.lib()
+    cb = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)(lambda n, u: None)
+    assert L.pat_set_device_allocator(ctypes.cast(cb, ctypes.c_void_p), None, None) == pat.PAT_ERR_INVALID_ARG
+    assert L.pat_set_device_allocator(None, None, None) == pat.PAT_OK
+    assert L.pat_get_stats(None, None) == pat.PAT_ERR_INVALID_ARG
