@@ -283,15 +283,20 @@ class Rig:
         self.l2_bytes = int(l2)
         self.plans, self.tr, self.img = [], [], []
         F = traces.shape[0]
-        for r in range(self.R):
-            p = pat.Plan(geom.n, geom.h, geom.origin, None, geom.sensors, geom.roi_index, geom.nt, geom.fs,
-                         geom.t0, weighting=pat.PAT_W_PAPER if weighting is None else weighting,
-                         max_batch=B if weighting is None or weighting < pat.PAT_W_PAPER_EXACT else 2 * B)
-            if variant:
-                pat.pat_set_gather_tuning(p.handle, *variant)
-            p.set_travel_times(tau)
-            if normals is not None:                            # universal BP: solid-angle table next to the delays
-                p.compute_solid_angle_weights(normals)
+        # buffers: one (traces, images) pair per plan; the warm-L2 rig has ONE plan and rotates three pairs, as a
+        # caller streaming frames does (consecutive calls must not share an image buffer to overlap, include/pat.h)
+        self.NB = 3 if warm_l2 else self.R
+        for r in range(self.NB):
+            if r < self.R:
+                p = pat.Plan(geom.n, geom.h, geom.origin, None, geom.sensors, geom.roi_index, geom.nt, geom.fs,
+                             geom.t0, weighting=pat.PAT_W_PAPER if weighting is None else weighting,
+                             max_batch=B if weighting is None or weighting < pat.PAT_W_PAPER_EXACT else 2 * B)
+                if variant:
+                    pat.pat_set_gather_tuning(p.handle, *variant)
+                p.set_travel_times(tau)
+                if normals is not None:                            # universal BP: solid-angle table next to the delays
+                    p.compute_solid_angle_weights(normals)
+                self.plans.append(p)
             sel = [(r * B + f) % F for f in range(B)]
             t = torch.from_numpy(np.ascontiguousarray(traces[sel]))
             if host:
@@ -300,28 +305,27 @@ class Rig:
             else:
                 self.tr.append(t.cuda())
                 self.img.append(torch.empty((B, geom.npix), dtype=torch.float32, device="cuda"))
-            self.plans.append(p)
         self.stream = torch.cuda.Stream()
         self.graphs, self.primed, self.use_graph = {}, False, not host
         self.last_regions = []
         torch.cuda.synchronize()
 
     def step(self, i):
-        r = i % self.R
-        self.plans[r].backproject(self.tr[r], self.img[r], self.B, self.stream)
+        r, q = i % self.R, i % self.NB
+        self.plans[r].backproject(self.tr[q], self.img[q], self.B, self.stream)
 
     def prime(self):
         """One direct call on every plan: the first call of a frame-count class builds its work list
         synchronously (pat.h), which must never land inside a timed region or a capture."""
         with self.torch.cuda.stream(self.stream):
-            for r in range(self.R):
+            for r in range(max(self.R, self.NB)):
                 self.step(r)
         self.torch.cuda.synchronize()
         self.primed = True
 
     def _graph(self, first, n):
         """CUDA graph of the n consecutive steps first .. first+n-1 of the plan rotation (cached)."""
-        key = (first % self.R, n)
+        key = (first % max(self.R, self.NB), n)
         g = self.graphs.get(key)
         if g is None:
             torch = self.torch

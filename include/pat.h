@@ -146,8 +146,22 @@ pat_status pat_set_travel_times(pat_plan *plan, const float *tau, int32_t sensor
  * pinned for the copies to be asynchronous).  Enqueues weighting pre-pass + gather (+ the
  * copies for host buffers) on `stream` and returns without synchronising -- except for the first
  * call with a given frame-count class (1, 2, 3-4, 5-8, 9-16, 17+) after the table changed, which
- * builds that class's work list (a few hundred KB of library-owned device memory, freed by
- * pat_destroy) and must therefore not happen inside a stream capture.
+ * builds that class's work list on the host (memory from the device-memory provider, size under "device memory"
+ * above: 0.7 MB for configs[1], ~0.6 GB and 0.7 s for the 34 GB table of configs[4]) and uploads it synchronously;
+ * that first call must therefore not happen inside a stream capture.
+ * A plan is driven from ONE stream at a time; traces and images must not overlap.
+ * Consecutive calls (cross-call overlap).  Inside a stream capture -- the way to run a ~10 us frame without paying
+ * a launch gap per kernel -- consecutive calls with DEVICE buffers are captured with explicit graph edges instead of
+ * a linear chain: the gather of call j hangs on the gather of call j-1 by a programmatic edge (its CTAs take over
+ * the SM slots that gather frees one by one) and the pre-pass of call j only on the gather of call j-3, so it runs
+ * while the two gathers before it are still busy (the plan rotates through three buffers of weighted traces).
+ * The library does this only when it can prove it safe at capture time: the capture's dependency set at the call
+ * is exactly the previous call's gather (nothing foreign in between), and the images/traces of the call do not
+ * overlap the images of the previous call (if they overlap those of the call before that -- a caller alternating
+ * between two image buffers -- the pre-pass waits for that gather instead).  In every other case, and always outside
+ * a capture, the call is ordered the ordinary way behind everything enqueued before it.  Work captured AFTER a call
+ * depends on that call's gather, whose completion implies the completion of every earlier call of the run.
+ * The results never depend on which way a call was captured.  pat_chained_calls counts the calls captured this way.
  * HOST buffers (the paper's timings include the transfers): the traces are copied on a
  * copy stream owned by the plan into one of two staging buffers and `stream` waits for that copy, so
  * the transfer of one call runs under the kernels of the previous call; everything is complete when

@@ -545,7 +545,7 @@ int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, f
         return launch_pre(ctx, prepass_exact_kernel<2>, dim3((unsigned)((quads + qpb - 1) / qpb), (unsigned)nsens, (unsigned)groups), 256,
                           traces, b, images, nsens, nt, nt4, ntb, nframes, log2_bp, npix, wp, wd, n_lo, quads, ready);
     }
-    if (bp <= 2) {
+    if (bp <= 2 || (!blocked && bp <= 8)) {
         const int64_t work = (int64_t)nsens * quads;
         int64_t blocks = (work + 256 * kSmallU - 1) / (256 * kSmallU);
         if (blocks > (int64_t)ctx.num_sms * 8) blocks = (int64_t)ctx.num_sms * 8;
@@ -558,6 +558,12 @@ int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, f
         }
         if (bp == 1)
             return launch_pre(ctx, prepass_small_kernel<1>, dim3((unsigned)blocks), 256, traces, b, images, nsens, nt, nt4,
+                              nframes, npix, wp, wd, t0fs, n_lo, quads, ready, ctx.pre_trace);
+        if (bp == 4)
+            return launch_pre(ctx, prepass_small_kernel<4>, dim3((unsigned)blocks), 256, traces, b, images, nsens, nt, nt4,
+                              nframes, npix, wp, wd, t0fs, n_lo, quads, ready, ctx.pre_trace);
+        if (bp == 8)
+            return launch_pre(ctx, prepass_small_kernel<8>, dim3((unsigned)blocks), 256, traces, b, images, nsens, nt, nt4,
                               nframes, npix, wp, wd, t0fs, n_lo, quads, ready, ctx.pre_trace);
         return launch_pre(ctx, prepass_small_kernel<2>, dim3((unsigned)blocks), 256, traces, b, images, nsens, nt, nt4,
                           nframes, npix, wp, wd, t0fs, n_lo, quads, ready, ctx.pre_trace);
