@@ -189,41 +189,64 @@ def eikonal_probe(geom):
             "speedup_vs_cpu_fmm": round((cpu / m) / (best / S), 2), "max_ulp_vs_cpu_fmm": int(d.max())}
 
 
-def conventional_probe(geom, traces, batches=(1, 32)):
+CONV_FLOPS_PER_UPDATE = 17      # the METHOD's arithmetic: delay 3 sub/mul pairs folded as 2 sub + 2 mul +
+                                # 1 add + sqrt + mul + sub + mul = 9, index map 4 (floor, k, a, 1 - a), interpolation 2 FMA = 4
+
+
+def conventional_probe(geom, traces, batches=(1, 32), sm_mhz=1965.0):
     """the conventional BP (tau = |r - s|/c0 computed in the gather) on the
-    same geometry.  No table stream, so the kernel is bound by arithmetic, not HBM; timed from a CUDA graph of
-    16 calls (traces resident, 4 MB/frame: they would fit L2 in any harness)."""
+    same geometry.  No table stream, so the kernel is bound by arithmetic, not HBM: the roofline is the method's
+    flops per update against the fp32 FMA peak (SMs x 128 lanes x 2 x clock).  Timed from a CUDA graph of 18 calls
+    over three image buffers (traces resident, 4 MB/frame: they would fit L2 in any harness).  Last row: the c0
+    sweep (one frame, 8 speeds per call -- the inner loop of the paper's automatic speed selection)."""
     import torch
     import paper_1501_03869_b200 as pat
+    sms = torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count
+    peak_tflops = sms * 128 * 2 * sm_mhz * 1e6 / 1e12
     out = []
-    for B in batches:
-        tr = torch.from_numpy(np.ascontiguousarray(np.resize(traces, (B,) + traces.shape[1:]))).cuda()
-        img = torch.empty((B, geom.npix), dtype=torch.float32, device="cuda")
-        plan = pat.Plan(geom.n, geom.h, geom.origin, geom.c_map, geom.sensors, geom.roi_index, geom.nt, geom.fs,
-                        geom.t0, max_batch=B)
+
+    def timed(plan, call, calls_per_graph, reps):
         st = torch.cuda.Stream()
         with torch.cuda.stream(st):
-            plan.backproject_conventional(tr, img, 1560.0, B, st)            # set-up outside the capture
+            call(0, st)                                              # set-up outside the capture
             st.synchronize()
             g = torch.cuda.CUDAGraph()
             with torch.cuda.graph(g, stream=st):
-                for _ in range(16):
-                    plan.backproject_conventional(tr, img, 1560.0, B, st)
+                for q in range(calls_per_graph):
+                    call(q, st)
             for _ in range(3):
                 g.replay()
             st.synchronize()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            reps = 20 if B == 1 else 4
             e0.record(st)
             for _ in range(reps):
                 g.replay()
             e1.record(st)
             st.synchronize()
-        ms = e0.elapsed_time(e1) / (16 * reps)
+        return e0.elapsed_time(e1) / (calls_per_graph * reps)
+
+    for B in batches:
+        tr = torch.from_numpy(np.ascontiguousarray(np.resize(traces, (B,) + traces.shape[1:]))).cuda()
+        imgs = [torch.empty((B, geom.npix), dtype=torch.float32, device="cuda") for _ in range(3)]
+        plan = pat.Plan(geom.n, geom.h, geom.origin, geom.c_map, geom.sensors, geom.roi_index, geom.nt, geom.fs,
+                        geom.t0, max_batch=B)
+        ms = timed(plan, lambda q, st: plan.backproject_conventional(tr, imgs[q % 3], 1560.0, B, st), 18, 20 if B == 1 else 4)
         upd = float(B) * geom.nsens * geom.npix
-        out.append({"B": B, "c0": 1560.0, "ms_per_frame": round(ms / B, 6), "gupd_s": round(upd / (ms * 1e-3) / 1e9, 1)})
-        del g
+        tf = upd * CONV_FLOPS_PER_UPDATE / (ms * 1e-3) / 1e12
+        out.append({"B": B, "c0": 1560.0, "ms_per_frame": round(ms / B, 6), "gupd_s": round(upd / (ms * 1e-3) / 1e9, 1),
+                    "roofline": {"bound": "alu", "achieved": round(tf, 2), "peak": round(peak_tflops, 1), "unit": "TFLOP/s",
+                                 "frac": round(tf / peak_tflops, 4), "flops_per_update": CONV_FLOPS_PER_UPDATE}})
         plan.close()
+    K = 8
+    c0s = np.linspace(1500.0, 1620.0, K).astype(np.float32)
+    tr1 = torch.from_numpy(np.ascontiguousarray(traces[0])).cuda()
+    imgs = [torch.empty((K, geom.npix), dtype=torch.float32, device="cuda") for _ in range(3)]
+    plan = pat.Plan(geom.n, geom.h, geom.origin, geom.c_map, geom.sensors, geom.roi_index, geom.nt, geom.fs, geom.t0, max_batch=1)
+    ms = timed(plan, lambda q, st: plan.backproject_conventional_sweep(tr1, imgs[q % 3], c0s, st), 18, 10)
+    upd = float(K) * geom.nsens * geom.npix
+    out.append({"sweep_speeds": K, "c0_range": [float(c0s[0]), float(c0s[-1])], "ms_per_call": round(ms, 6),
+                "ms_per_image": round(ms / K, 6), "gupd_s": round(upd / (ms * 1e-3) / 1e9, 1)})
+    plan.close()
     return out
 
 
@@ -639,7 +662,7 @@ def run_ours(args):
             print(json.dumps({"exact_time_weighting": exact_time_probe(g1, tau1, tr1, peak_gbs, batches=(args.batch or 1,))}))
         else:
             g1, _, tr1 = prepare_inputs(k, args.reduced, 1)
-            print(json.dumps({"conventional_bp": conventional_probe(g1, tr1, batches=(args.batch or 1,))}))
+            print(json.dumps({"conventional_bp": conventional_probe(g1, tr1, batches=(args.batch or 1,), sm_mhz=sm_max)}))
         return 0
     B = args.batch or geom0.batch
     do_sweep = (not args.no_sweep) and world == 1 and k in (1, 2) and not args.batch
@@ -689,7 +712,7 @@ def run_ours(args):
                 "algorithmic_bytes_over_time_vs_hbm_peak": round(mw["step_hbm_frac"], 4)}
     if do_sweep:
         eik = eikonal_probe(geom)
-        conv = conventional_probe(geom, traces)
+        conv = conventional_probe(geom, traces, sm_mhz=sm_max)
         exact = exact_time_probe(geom, tau, traces, peak_gbs)
         ubp = universal_bp_probe(geom, tau, traces, peak_gbs)
     sampler.stop_flag = True

@@ -187,6 +187,21 @@ pat_status pat_backproject(pat_plan *plan, const float *traces, float *images,
 pat_status pat_backproject_conventional(pat_plan *plan, const float *traces, float *images,
                                         int32_t nframes, float c0, void *stream);
 
+/* pat_backproject_conventional_sweep -- SURVEY.md 8(f) NEXT-3, "a c0 sweep (autofocus-style)": the paper picks the
+ * conventional BP's speed, c0 = 1560 m/s, "by an automatic sound speed selection", i.e. by reconstructing
+ * with many candidate speeds.  One call reconstructs ONE frame with nc0 speeds:
+ *     images[q][j] = pat_backproject_conventional(traces, c0[q])[j]        q = 0 .. nc0-1
+ * bit-for-bit the same delays (tau = sqrt(d2) * (1/c0[q]), then the time -> sample map), but the distance of a
+ * (pixel, sensor) pair is formed once for all speeds and the trace windows -- sized for the envelope of the delays
+ * over [min c0, max c0] -- are staged once: the speeds play the role of the frame axis.
+ *   traces  DEVICE fp32 [nsens][nt] (one frame)      images  DEVICE fp32 [nc0][npix]
+ *   c0      HOST fp32 [nc0], finite and > 0, 1 <= nc0 <= PAT_MAX_SWEEP; read before the call returns
+ * The first call with a new (min c0, max c0) builds row ranges and a work list (synchronises `stream`).
+ * Errors as pat_backproject_conventional; host buffers, _EXACT weightings, pixel weights -> PAT_ERR_UNSUPPORTED. */
+#define PAT_MAX_SWEEP 16
+pat_status pat_backproject_conventional_sweep(pat_plan *plan, const float *traces, float *images,
+                                              const float *c0, int32_t nc0, void *stream);
+
 /* pat_set_roi_mask -- PAPER.md:81: "a specific region of interest can be selected for reconstruction to
  * further reduce the reconstruction time" -- without touching the uploaded table.
  *   mask   HOST uint8 [npix] in roi_index order, non-zero = reconstruct; NULL = all pixels again.

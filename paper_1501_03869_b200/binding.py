@@ -107,6 +107,8 @@ def lib():
     L.pat_set_roi_mask.argtypes = [vp, vp]
     L.pat_backproject_conventional.restype = ctypes.c_int
     L.pat_backproject_conventional.argtypes = [vp, vp, vp, i32, ctypes.c_float, vp]
+    L.pat_backproject_conventional_sweep.restype = ctypes.c_int
+    L.pat_backproject_conventional_sweep.argtypes = [vp, vp, vp, vp, i32, vp]
     L.pat_eikonal_travel_times_device.restype = ctypes.c_int
     L.pat_eikonal_travel_times_device.argtypes = [gp, vp, vp, i32, vp, i64, i32, i32, vp, i32,
                                                   ctypes.POINTER(i32), vp]
@@ -236,6 +238,13 @@ def pat_backproject_conventional(plan, traces, images, nframes, c0, stream=None)
     """Eq. 7 with tau = |r - s| / c0 computed in the kernel."""
     return _check(plan, lib().pat_backproject_conventional(plan, _addr(traces), _addr(images), nframes,
                                                            float(c0), _stream(stream)))
+
+
+def pat_backproject_conventional_sweep(plan, traces, images, c0, stream=None):
+    """One frame, len(c0) speeds: images[q] = conventional BP with c0[q] (the c0 selection's inner loop)."""
+    c0 = np.ascontiguousarray(c0, dtype=np.float32)
+    return _check(plan, lib().pat_backproject_conventional_sweep(plan, _addr(traces), _addr(images), _addr(c0),
+                                                                 int(c0.size), _stream(stream)))
 
 
 def pat_get_trace_window(plan):
@@ -377,6 +386,9 @@ class Plan:
     def backproject_conventional(self, traces, images, c0, nframes=None, stream=None):
         nframes = int(traces.shape[0]) if nframes is None else nframes
         return pat_backproject_conventional(self.handle, traces, images, nframes, c0, stream)
+
+    def backproject_conventional_sweep(self, traces, images, c0, stream=None):
+        return pat_backproject_conventional_sweep(self.handle, traces, images, c0, stream)
 
     def set_pixel_weights(self, w, sensor_begin=0, count=None, stream=None):
         return pat_set_pixel_weights(self.handle, w, sensor_begin, count, stream)

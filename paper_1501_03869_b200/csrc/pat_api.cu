@@ -429,7 +429,7 @@ pat_status get_schedule(pat_plan *p, int bp, bool onfly, PatSchedule **out) {
 
 // Conventional BP set-up: node coordinates of every tile slot and the sensors on the device (once), and the
 // k-range of every (tile, sensor) row for this c0 (a kernel with the gather's own arithmetic; synchronises).
-pat_status ensure_onfly(pat_plan *p, float c0, void *stream, PatOnfly *out) {
+pat_status ensure_onfly(pat_plan *p, float c0, float c0_hi, void *stream, PatOnfly *out) {   // c0 <= c0_hi: a sweep's range
     const int64_t slots = p->dims.ntiles * kTilePix;
     const int32_t S = p->dims.nsens;
     cudaStream_t st = (cudaStream_t)stream;
@@ -463,7 +463,7 @@ pat_status ensure_onfly(pat_plan *p, float c0, void *stream, PatOnfly *out) {
     }
     out->pix = p->d_pix; out->sens = p->d_sens; out->pix_stride = slots;
     out->inv_c0 = 1.0f / c0; out->t0 = p->t0; out->fs = p->fs; out->ndim = p->grid.ndim;
-    if (p->onfly_c0 != c0 || p->onfly_meta.empty()) {
+    if (p->onfly_c0 != c0 || p->onfly_c0_hi != c0_hi || p->onfly_meta.empty()) {
         const int64_t nrows = p->dims.ntiles * S;
         // scratch for the row ranges: the workspace's meta array is the table path's; same size, own block
         PatDevBuf mbuf;
@@ -477,9 +477,46 @@ pat_status ensure_onfly(pat_plan *p, float c0, void *stream, PatOnfly *out) {
         try { p->onfly_meta.resize((size_t)nrows * 2); } catch (...) { cudaStreamSynchronize(st); plan_free(p, &mbuf); return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
         if (!le) e = cudaMemcpyAsync(p->onfly_meta.data(), d_meta, (size_t)nrows * 8, cudaMemcpyDeviceToHost, st);
         if (!le && e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (!le && e == cudaSuccess && c0_hi != c0) {
+            // a sweep over [c0, c0_hi]: the delay of a (pixel, sensor) pair falls monotonically with the speed, so the
+            // samples it can touch over the whole range lie between its k at c0_hi and its k at c0 -- the envelope
+            // of the two row ranges; a row is all-valid over the range if it is at both ends
+            std::vector<int32_t> hi_meta;
+            try { hi_meta.resize((size_t)nrows * 2); } catch (...) { le = (int)cudaErrorMemoryAllocation; }
+            PatOnfly o2 = *out;
+            o2.inv_c0 = 1.0f / c0_hi;
+            if (!le) le = pat_launch_onfly_meta(ctx, o2, S, d_meta, nrows, p->dims.nt);
+            ++p->launches;
+            if (!le) e = cudaMemcpyAsync(hi_meta.data(), d_meta, (size_t)nrows * 8, cudaMemcpyDeviceToHost, st);
+            if (!le && e == cudaSuccess) e = cudaStreamSynchronize(st);
+            if (!le && e == cudaSuccess) {
+                // onfly_meta holds the ranges at the LOWEST speed (longest delays), hi_meta at the highest.  A pixel
+                // beyond the record at the lowest speed comes into it somewhere in between with k up to nt-2, and
+                // (only if t0 > 0) a pixel before the record at the highest speed enters it with k from 0.
+                const int32_t kend = p->dims.nt - 2;
+                const bool early = p->t0 > 0.0f;
+                for (int64_t r = 0; r < nrows; ++r) {
+                    int32_t &k0 = p->onfly_meta[(size_t)2 * r], &k1 = p->onfly_meta[(size_t)2 * r + 1];
+                    const int32_t h0 = hi_meta[(size_t)2 * r], h1 = hi_meta[(size_t)2 * r + 1];
+                    const int32_t a1 = k1 < 0 ? -1 : (k1 & 0x3FFFFFFF), b1 = h1 < 0 ? -1 : (h1 & 0x3FFFFFFF);
+                    const bool va = a1 >= k0, vb = b1 >= h0;                 // any valid pixel at the low / high speed
+                    const bool alla = va && (k1 >> 30 & 1), allb = vb && (h1 >> 30 & 1);
+                    if (!vb && !early) { k0 = INT32_MAX; k1 = -1; continue; }   // beyond the record at every speed
+                    int32_t lo = vb ? h0 : INT32_MAX, hi = va ? a1 : -1;
+                    if (va) lo = std::min(lo, k0);
+                    if (vb) hi = std::max(hi, b1);
+                    if (!alla) hi = kend;
+                    if (!allb && early) lo = 0;
+                    if (hi < lo) { k0 = INT32_MAX; k1 = -1; continue; }
+                    k0 = lo;
+                    k1 = hi | (alla && allb ? 1 << 30 : 0);
+                }
+            }
+        }
         plan_free(p, &mbuf);
         if (le || e != cudaSuccess) { p->onfly_meta.clear(); return cuda_fail(p, le ? le : (int)e, "conventional BP row ranges"); }
         p->onfly_c0 = c0;
+        p->onfly_c0_hi = c0_hi;
         needed_samples(p->onfly_meta, p->dims.nt, &p->onfly_lo, &p->onfly_hi);
         // work lists of the previous c0 are stale
         for (size_t q = 0; q < p->schedules.size();) {
@@ -722,7 +759,7 @@ extern "C" pat_status pat_set_travel_times(pat_plan *p, const float *tau, int32_
 }
 
 static pat_status backproject_impl(pat_plan *p, const float *traces, float *images, int32_t nframes, void *stream,
-                                   bool conventional, float c0);
+                                   bool conventional, float c0, const float *sweep_c0 = nullptr, int32_t nsweep = 0);
 
 extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *images,
                                       int32_t nframes, void *stream) {
@@ -737,9 +774,22 @@ extern "C" pat_status pat_backproject_conventional(pat_plan *p, const float *tra
     return backproject_impl(p, traces, images, nframes, stream, true, c0);
 }
 
-static pat_status backproject_impl(pat_plan *p, const float *traces, float *images, int32_t nframes, void *stream,
-                                   bool conventional, float c0) {
+extern "C" pat_status pat_backproject_conventional_sweep(pat_plan *p, const float *traces, float *images,
+                                                         const float *c0, int32_t nc0, void *stream) {
     if (!p) return PAT_ERR_INVALID_ARG;
+    if (!c0 || nc0 < 1 || nc0 > PAT_MAX_SWEEP) return fail(p, PAT_ERR_INVALID_ARG, "c0 is NULL or nc0 outside [1, PAT_MAX_SWEEP]");
+    for (int32_t q = 0; q < nc0; ++q)
+        if (!(c0[q] > 0.0f) || !std::isfinite(c0[q])) return fail(p, PAT_ERR_INVALID_ARG, "every c0 must be finite and > 0");
+    if (p->sensors.empty()) return fail(p, PAT_ERR_BAD_STATE, "plan was created without sensor_xyz");
+    if (p->exact) return fail(p, PAT_ERR_UNSUPPORTED, "the sweep is not available with the _EXACT weightings");
+    if (p->d_w_t) return fail(p, PAT_ERR_UNSUPPORTED, "the sweep is not combined with pixel weights");
+    return backproject_impl(p, traces, images, 1, stream, true, c0[0], c0, nc0);
+}
+
+static pat_status backproject_impl(pat_plan *p, const float *traces, float *images, int32_t nframes, void *stream,
+                                   bool conventional, float c0, const float *sweep_c0, int32_t nsweep) {
+    if (!p) return PAT_ERR_INVALID_ARG;
+    const int32_t nimages = nsweep > 0 ? nsweep : nframes;      // a sweep: ONE frame of traces, one image per speed
     if (nframes < 0 || nframes > p->dims.max_batch)
         return fail(p, PAT_ERR_INVALID_ARG, "nframes outside [0, max_batch]");
     const int32_t nch = p->exact ? 2 * nframes : nframes;       // exact-time weightings: two channels per frame
@@ -754,6 +804,7 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
     if (td != id) return fail(p, PAT_ERR_INVALID_ARG, "traces and images must both be host or both device");
     if (td && ((((uintptr_t)traces) | ((uintptr_t)images)) & 15u))
         return fail(p, PAT_ERR_INVALID_ARG, "device traces/images must be 16-byte aligned");
+    if (nsweep > 0 && !td) return fail(p, PAT_ERR_UNSUPPORTED, "the sweep takes DEVICE buffers");
 
     cudaStream_t st = (cudaStream_t)stream;
     const PatDims &d = p->dims;
@@ -763,8 +814,12 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
     bool piped = false;
     PatOnfly onfly;
     if (conventional) {      // geometry + k-ranges for this c0 (first use: builds them, synchronous)
-        pat_status os = ensure_onfly(p, c0, stream, &onfly);
+        float c_lo = c0, c_hi = c0;
+        for (int32_t q = 0; q < nsweep; ++q) { c_lo = std::min(c_lo, sweep_c0[q]); c_hi = std::max(c_hi, sweep_c0[q]); }
+        pat_status os = ensure_onfly(p, c_lo, c_hi, stream, &onfly);
         if (os != PAT_OK) return os;
+        onfly.nsweep = nsweep;
+        for (int32_t q = 0; q < nsweep; ++q) onfly.sweep_inv_c0[q] = 1.0f / sweep_c0[q];
     }
     if (!td) {
         d_tr = (const float *)(p->ws + (slot ? p->lay.traces2 : p->lay.traces));
@@ -809,7 +864,7 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
     const bool prof = p->profiling == 1 && p->prof_events.size() < 3u * 65536u;
     PatLaunchCtx ctx{stream, p->num_sms, p->use_pdl && !prof};
     ctx.high_priority = p->prio_high;
-    const size_t ibytes = (size_t)nframes * d.npix * sizeof(float);
+    const size_t ibytes = (size_t)nimages * d.npix * sizeof(float);
     const bool do_gather = sc->grid_x > 0 && p->profiling != 3;
     const bool do_pre = p->profiling != 2;
     // launch chain (see the top of this file): only for device buffers inside a capture
@@ -865,7 +920,8 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
         e = pat_launch_prepass(ctx, d_tr, bw, d_img, d.nsens, d.nt, p->nt4, nframes, bp, d.npix, p->wp, p->wd, t0fs, p->exact,
                                p->window_prepass ? (conventional ? p->onfly_lo : p->need_lo) : 0,
                                p->window_prepass ? (conventional ? p->onfly_hi : p->need_hi) : INT32_MAX,
-                               do_gather && !cp.chained ? sync : nullptr);   // chained: a full edge orders P before G
+                               do_gather && !cp.chained ? sync : nullptr,    // chained: a full edge orders P before G
+                               (int64_t)nimages * d.npix);
         if (e) return cuda_fail(p, e, "pre-pass launch");
         ++p->launches;
         if (cp.capture_id) capture_deps(st, &cid, &node_pre);

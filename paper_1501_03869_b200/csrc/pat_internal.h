@@ -73,6 +73,8 @@ struct PatOnfly {
     int64_t pix_stride = 0;
     float inv_c0 = 0, t0 = 0, fs = 0;
     int32_t ndim = 2;
+    int32_t nsweep = 0;                 // > 0: pat_backproject_conventional_sweep, one image per speed
+    float sweep_inv_c0[PAT_MAX_SWEEP] = {};
 };
 
 // Device memory the library asks for on its own goes through the caller's provider (alloc.cu).
@@ -145,7 +147,7 @@ struct pat_plan {
     // conventional BP (pat_backproject_conventional): geometry on the device, k-ranges for the current c0
     std::vector<int32_t> host_perm;   // tile slot -> ROI position (-1 = padding)
     float *d_pix = nullptr, *d_sens = nullptr;
-    float onfly_c0 = 0;
+    float onfly_c0 = 0, onfly_c0_hi = 0;   // speed (range, for a sweep) the row ranges below were computed for
     std::vector<int32_t> onfly_meta;
     // pat_set_pixel_weights / pat_compute_solid_angle_weights: per-(sensor, pixel) factors, tile-major like u_t
     float *d_w_t = nullptr;           // library-owned [ntiles][nsens][256], NULL = no weights
@@ -183,8 +185,9 @@ int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, f
                        int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp,
                        int64_t npix, float wp, float wd, float t0fs, bool exact = false,
                        int32_t n_lo = 0, int32_t n_hi = INT32_MAX,    // only samples [n_lo, n_hi) of b are needed
-                       uint32_t *ready = nullptr);                    // [0]: every block counts itself when its part of b / images is
+                       uint32_t *ready = nullptr,                     // [0]: every block counts itself when its part of b / images is
                                                                       // written, the last one raises the flag [32]
+                       int64_t nzero = -1);                           // image floats to zero (-1: nframes*npix)
 
 // Measurement only (pat_set_profiling mode 4): stream a_bytes + c_bytes in, nout floats out.
 int pat_launch_stream_probe(const PatLaunchCtx &ctx, const void *a, int64_t a_bytes, const void *c, int64_t c_bytes,

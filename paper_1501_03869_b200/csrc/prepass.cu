@@ -283,12 +283,12 @@ prepass_il16_kernel(const float *__restrict__ traces, float *__restrict__ b, flo
 constexpr int kB1Threads = 128, kB1U = 4;
 __global__ void __launch_bounds__(kB1Threads, 8)
 prepass_b1_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
-                  int32_t nsens, int32_t nt, int32_t nt4, int64_t npix, float wp, float wd, float t0fs,
+                  int32_t nsens, int32_t nt, int32_t nt4, int64_t nzero, float wp, float wd, float t0fs,
                   int32_t n_lo, int32_t quads, uint32_t *ready, unsigned long long *trace) {
     asm volatile("griddepcontrol.launch_dependents;");
     if (trace && blockIdx.x == 0 && threadIdx.x == 0) trace[0] = pre_gtime();
     const uint32_t gid = blockIdx.x * kB1Threads + threadIdx.x, nthr = gridDim.x * kB1Threads;
-    for (uint32_t q = gid; q < (uint32_t)npix; q += nthr) images[q] = 0.0f;
+    for (uint32_t q = gid; q < (uint32_t)nzero; q += nthr) images[q] = 0.0f;
     const uint32_t total = (uint32_t)nsens * (uint32_t)quads;
     for (uint32_t q = gid; q < total; q += kB1U * nthr) {
         float w[kB1U][6];
@@ -520,7 +520,8 @@ static int launch_pre(const PatLaunchCtx &ctx, void (*kern)(KArgs...), dim3 grid
 int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, float *images,
                        int32_t nsens, int32_t nt, int32_t nt4, int32_t nframes, int32_t bp,
                        int64_t npix, float wp, float wd, float t0fs, bool exact, int32_t n_lo, int32_t n_hi,
-                       uint32_t *ready) {
+                       uint32_t *ready, int64_t nzero) {
+    if (nzero < 0) nzero = npix * nframes;
     // Only samples [n_lo, n_hi) of b can be read by a valid pixel (the caller's k-ranges; whole quads): the rest
     // of b is left as it is.  The blocked layout works in whole 32-sample blocks.
     const int32_t ntb = (nt + 31) / 32;
@@ -550,15 +551,15 @@ int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, f
         int64_t blocks = (work + 256 * kSmallU - 1) / (256 * kSmallU);
         if (blocks > (int64_t)ctx.num_sms * 8) blocks = (int64_t)ctx.num_sms * 8;
         if (blocks < 1) blocks = 1;
-        if (bp == 1 && (nt & 3) == 0 && nframes == 1 && work < (1ll << 31) && npix < (1ll << 32)) {
+        if (bp == 1 && (nt & 3) == 0 && nframes == 1 && work < (1ll << 31) && nzero < (1ll << 32)) {
             int64_t nb = (work + kB1Threads * kB1U - 1) / (kB1Threads * kB1U);   // one wave on configs[1] (130 blocks)
             if (nb > (int64_t)ctx.num_sms * 8) nb = (int64_t)ctx.num_sms * 8;
             return launch_pre(ctx, prepass_b1_kernel, dim3((unsigned)std::max<int64_t>(nb, 1)), kB1Threads, traces, b, images,
-                              nsens, nt, nt4, npix, wp, wd, t0fs, n_lo, quads, ready, ctx.pre_trace);
+                              nsens, nt, nt4, nzero, wp, wd, t0fs, n_lo, quads, ready, ctx.pre_trace);
         }
-        if (bp == 1)
+        if (bp == 1)                                     // (zeroes npix*nframes floats: nframes is 1 here)
             return launch_pre(ctx, prepass_small_kernel<1>, dim3((unsigned)blocks), 256, traces, b, images, nsens, nt, nt4,
-                              nframes, npix, wp, wd, t0fs, n_lo, quads, ready, ctx.pre_trace);
+                              nframes, nframes == 1 ? nzero : npix, wp, wd, t0fs, n_lo, quads, ready, ctx.pre_trace);
         if (bp == 4)
             return launch_pre(ctx, prepass_small_kernel<4>, dim3((unsigned)blocks), 256, traces, b, images, nsens, nt, nt4,
                               nframes, npix, wp, wd, t0fs, n_lo, quads, ready, ctx.pre_trace);

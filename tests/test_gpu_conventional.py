@@ -132,3 +132,65 @@ def test_conventional_host_buffers_transfer_only_the_reachable_samples():
             assert_parity(img.numpy(), ref, "conventional, host buffers, c0=%g" % c0)
     finally:
         plan.close()
+
+
+# ---- the c0 sweep ("+ a c0 sweep (autofocus-style)") ---------------------
+def _sweep(plan, traces1, c0s, npix):
+    import torch
+    img = torch.full((len(c0s), npix), float("nan"), dtype=torch.float32, device="cuda")
+    plan.backproject_conventional_sweep(torch.from_numpy(np.ascontiguousarray(traces1)).cuda(), img, c0s)
+    torch.cuda.synchronize()
+    return img.cpu().numpy()
+
+
+@pytest.mark.parametrize("k,reduced,c0s,mode", [
+    (0, False, [1480.0, 1520.0, 1560.0, 1600.0, 1640.0], 1),
+    (1, False, [1560.0], 1),
+    (1, False, list(np.linspace(1450.0, 1650.0, 16)), 2),
+    (4, True, [1500.0, 1540.0, 1580.0], 0),
+])
+def test_c0_sweep_equals_one_oracle_run_per_speed(k, reduced, c0s, mode):
+    """images[q] of ONE sweep call = the oracle's conventional BP with c0[q] (K oracle runs), same tolerance; speeds in
+    any order, the extremes define the staged windows."""
+    geom = W.make_geometry(k, reduced)
+    rng = np.random.default_rng(300 + k)
+    traces = rng.standard_normal((1, geom.nsens, geom.nt)).astype(np.float32)
+    c0s = list(c0s)
+    rng.shuffle(c0s)
+    plan = _plan(geom, 1, mode)
+    try:
+        got = _sweep(plan, traces[0], c0s, geom.npix)
+        for q, c0 in enumerate(c0s):
+            tau = oracle.tau_conventional(geom.n, geom.h, geom.origin, geom.sensors, geom.roi_index, c0)
+            ref = oracle.backproject(tau, traces, geom.fs, geom.t0, mode)
+            assert_parity(got[q:q + 1], ref, "sweep k=%d c0=%g" % (k, c0))
+        # a single-speed call on the same plan afterwards (row ranges and work lists are rebuilt for it)
+        c0 = c0s[0]
+        tau = oracle.tau_conventional(geom.n, geom.h, geom.origin, geom.sensors, geom.roi_index, c0)
+        assert_parity(_run(plan, traces, c0, geom.npix), oracle.backproject(tau, traces, geom.fs, geom.t0, mode), "after the sweep")
+    finally:
+        plan.close()
+
+
+def test_c0_sweep_with_speeds_that_push_delays_out_of_the_record_and_argument_errors():
+    """A very low speed moves most delays past the end of the record (those terms are 0, R7); bad arguments."""
+    import torch
+    import paper_1501_03869_b200 as pat
+    geom = W.make_geometry(0)
+    rng = np.random.default_rng(31)
+    traces = rng.standard_normal((1, geom.nsens, geom.nt)).astype(np.float32)
+    c0s = [600.0, 1540.0, 9000.0]
+    plan = _plan(geom, 1)
+    try:
+        got = _sweep(plan, traces[0], c0s, geom.npix)
+        for q, c0 in enumerate(c0s):
+            tau = oracle.tau_conventional(geom.n, geom.h, geom.origin, geom.sensors, geom.roi_index, c0)
+            assert_parity(got[q:q + 1], oracle.backproject(tau, traces, geom.fs, geom.t0, 1), "sweep c0=%g" % c0)
+        tr = torch.from_numpy(traces[0]).cuda()
+        img = torch.empty((17, geom.npix), dtype=torch.float32, device="cuda")
+        for bad in ([], [1500.0] * 17, [1500.0, -1.0], [float("nan")]):
+            with pytest.raises(pat.PatError) as ei:
+                plan.backproject_conventional_sweep(tr, img, bad)
+            assert ei.value.status == pat.PAT_ERR_INVALID_ARG
+    finally:
+        plan.close()
