@@ -505,7 +505,8 @@ def measure(geom, tau, traces, B, steps, warmup, variant, dist, peak_gbs, sm_mhz
     if do_e2e:
         hrig = Rig(geom, tau, traces, B, variant, host=True)
         hrig.prime()                                     # every plan's first call (work-list build) is set-up
-        n_e2e = max(2 * hrig.R, min(steps, 200))
+        n_e2e = max(2 * hrig.R, 200)                     # its own region length, whatever --steps is: in a 20-call
+                                                         # region a third is pipeline fill (first H2D, last D2H uncovered)
         ms_h = time_steps(hrig, n_e2e, min(warmup, 10), dist)
         out["e2e_gupd_s"] = upd * n_e2e / (ms_h * 1e-3) / 1e9
         out["e2e_ms_per_step"] = ms_h / n_e2e
