@@ -325,6 +325,34 @@ pat_status pat_eikonal_travel_times_device(const pat_grid *grid, const float *c_
 pat_status pat_compute_travel_times_gpu(pat_plan *plan, int32_t max_rounds, int32_t *rounds_out,
                                         void *stream);
 
+/* ---- the entry point that allocates nothing -------------------------------------------------------------
+ * Eq. 7 with the sample-time weightings, for callers that cannot call cudaMalloc (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid it): no plan, no workspace, no allocator.  The only
+ * scratch of the path -- the weighted traces b the pre-pass writes and the gather reads -- is a file-scope
+ * __device__ array of PAT_STATIC_MAX_SAMPLES floats (4 MiB) that every GPU holds from the moment it loads the
+ * library until the process exits.  The call enqueues two kernels on `stream` and returns; it calls no cudaMalloc,
+ * cudaFree or other allocating routine, copies nothing, and does not synchronise.
+ *   tau      DEVICE fp32 [nsens][npix], seconds, row-major as pat_set_travel_times takes it (not retained)
+ *   traces   DEVICE fp32 [nframes][nsens][nt]
+ *   images   DEVICE fp32 [nframes][npix], written (not accumulated): needs no zeroing
+ *   u = fl32(fl32(tau - t0)*fs), k = floor(u), a = u - k, terms with !(0 <= u < nt-1) contribute 0 -- the index rule
+ *   and the per-term arithmetic of pat_backproject; the sum over sensors runs in another order (fp32), so the two
+ *   agree within the tolerance of DESIGN.md section 3, not bit for bit.  A plain variant of the kernels: the tuned
+ *   table layout and pipeline of the plan path are not here (expect a few times pat_backproject's step time).
+ * Limit: nframes*nsens*nt <= PAT_STATIC_MAX_SAMPLES (the paper-scale frame, 512 x 2048, fits exactly); beyond it ->
+ * PAT_ERR_INVALID_ARG with the numbers in the error text.  The array is shared by all calls on a device and keeps
+ * the last call's contents; every call overwrites the part it reads, nothing in it must start at zero.  Calls that
+ * OVERLAP on the GPU (different streams) race on the array; calls on one stream are ordered.
+ * Errors: NULL / host pointers, sizes <= 0, nt < 2, non-finite fs or t0 -> PAT_ERR_INVALID_ARG; _EXACT weightings
+ * -> PAT_ERR_UNSUPPORTED; not an sm_100 device -> PAT_ERR_UNSUPPORTED; CUDA failure -> PAT_ERR_CUDA.  The text is
+ * returned by pat_backproject_static_last_error (per thread; never NULL). */
+#define PAT_STATIC_MAX_SAMPLES (1 << 20)
+pat_status pat_backproject_static(const float *tau, const float *traces, float *images, int32_t nsens,
+                                  int64_t npix, int32_t nt, int32_t nframes, float fs, float t0,
+                                  pat_weighting weighting, void *stream);
+int64_t pat_backproject_static_max_samples(void);
+const char *pat_backproject_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -13,6 +13,7 @@ from .binding import (PAT_OK, PAT_ERR_INVALID_ARG, PAT_ERR_BAD_STATE, PAT_ERR_CU
                       pat_compute_travel_times, pat_set_profiling, pat_get_profile,
                       pat_eikonal_travel_times_device, pat_compute_travel_times_gpu,
                       pat_backproject_conventional, pat_backproject_conventional_sweep, pat_set_roi_mask, pat_set_pixel_weights,
-                      pat_compute_solid_angle_weights, pat_get_trace_window, Plan)
+                      pat_compute_solid_angle_weights, pat_get_trace_window, Plan,
+                      pat_backproject_static, pat_backproject_static_max_samples, pat_backproject_static_last_error)
 
 __all__ = [n for n in dir() if n.startswith(("pat_", "PAT_", "Pat", "Plan", "lib"))]

@@ -114,6 +114,12 @@ def lib():
                                                   ctypes.POINTER(i32), vp]
     L.pat_compute_travel_times_gpu.restype = ctypes.c_int
     L.pat_compute_travel_times_gpu.argtypes = [vp, i32, ctypes.POINTER(i32), vp]
+    L.pat_backproject_static.restype = ctypes.c_int
+    L.pat_backproject_static.argtypes = [vp, vp, vp, i32, i64, i32, i32, f32, f32, i32, vp]
+    L.pat_backproject_static_max_samples.restype = i64
+    L.pat_backproject_static_max_samples.argtypes = []
+    L.pat_backproject_static_last_error.restype = ctypes.c_char_p
+    L.pat_backproject_static_last_error.argtypes = []
     _lib = L
     return L
 
@@ -342,6 +348,25 @@ def pat_compute_travel_times_gpu(plan, max_rounds=0, stream=None):
     r = ctypes.c_int32()
     _check(plan, lib().pat_compute_travel_times_gpu(plan, int(max_rounds), ctypes.byref(r), _stream(stream)))
     return r.value
+
+
+def pat_backproject_static_max_samples():
+    return int(lib().pat_backproject_static_max_samples())
+
+
+def pat_backproject_static_last_error():
+    return lib().pat_backproject_static_last_error().decode()
+
+
+def pat_backproject_static(tau, traces, images, nsens, npix, nt, nframes, fs, t0=0.0, weighting=PAT_W_PAPER,
+                           stream=None):
+    """The entry point that allocates nothing (include/pat.h): device pointers in, images out, scratch in a
+    static __device__ array of pat_backproject_static_max_samples() floats."""
+    st = lib().pat_backproject_static(_addr(tau), _addr(traces), _addr(images), int(nsens), int(npix), int(nt),
+                                      int(nframes), float(fs), float(t0), int(weighting), _stream(stream))
+    if st != PAT_OK:
+        raise PatError(st, pat_backproject_static_last_error())
+    return st
 
 
 class Plan:
