@@ -159,34 +159,49 @@ def prepare_inputs(k, reduced, nframes, frame0=0):
     return geom, tau, traces
 
 
-def eikonal_probe(geom):
+EIK_FLOPS_PER_UPDATE = {2: 14, 3: 26}   # fp64 operations of one upwind update as written in csrc/eikonal.cu (min/compare
+                                        # per axis, sort, one- / two- / three-axis solve incl. the square root)
+FP64_PEAK_TFLOPS = 40.0                 # NVIDIA's B200 data-sheet FP64 figure; the guides state none (context only)
+
+
+def eikonal_probe(geom, sample=None, cpu_sample=64, reps=3):
     """SURVEY.md 8(f) NEXT-2, off the timed path: the travel-time table of this geometry solved on the GPU
     (fast sweeping, csrc/eikonal.cu) beside the library's CPU fast marching on the host cores (a sample of
-    the sensors), wall clock, and how far the two tables are apart."""
+    the sensors), wall clock, and how far the two tables are apart.  sample = n: only the first n sensors are
+    solved (one chunk of a table that is solved chunk by chunk anyway); ms/sensor is what scales."""
     import torch
     import paper_1501_03869_b200 as pat
     grid = pat.PatGrid.make(geom.n, geom.h, geom.origin)
     cm = np.ascontiguousarray(geom.c_map, dtype=np.float32).ravel()
     S = geom.nsens
-    out = torch.empty((S, geom.npix), dtype=torch.float32, device="cuda")
+    n = S if sample is None else min(S, sample)
+    out = torch.empty((n, geom.npix), dtype=torch.float32, device="cuda")
     best, rounds = None, 0
-    for _ in range(3):
+    for _ in range(reps):
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        rounds = pat.pat_eikonal_travel_times_device(grid, cm, geom.sensors, S, geom.roi_index, geom.npix, 0, S, out)
+        rounds = pat.pat_eikonal_travel_times_device(grid, cm, geom.sensors, S, geom.roi_index, geom.npix, 0, n, out)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
         best = dt if best is None else min(best, dt)
-    m = min(S, 64)
+    m = min(n, cpu_sample)
     tau = np.empty((m, geom.npix), dtype=np.float32)
     t0 = time.perf_counter()
     pat.pat_fmm_travel_times(grid, cm, geom.sensors, S, geom.roi_index, geom.npix, 0, m, 1, tau, 0)
     cpu = time.perf_counter() - t0
     d = np.abs(out[:m].cpu().numpy().view(np.int32).astype(np.int64) - tau.view(np.int32).astype(np.int64))
-    return {"workload": "%d sensors on the %s grid (first-order upwind, fp64)" % (S, "x".join(str(v) for v in geom.n)),
-            "gpu_s": round(best, 4), "gpu_ms_per_sensor": round(best * 1e3 / S, 4), "rounds": int(rounds),
+    nodes = float(np.prod(geom.n))
+    ndim = len(geom.n)
+    upd = n * nodes * rounds * (1 << ndim)                 # node updates: every pass of every round visits every node
+    tf = upd * EIK_FLOPS_PER_UPDATE[ndim] / best / 1e12
+    return {"workload": "%d of %d sensors on the %s grid (first-order upwind, fp64)" % (n, S, "x".join(str(v) for v in geom.n)),
+            "gpu_s": round(best, 4), "gpu_ms_per_sensor": round(best * 1e3 / n, 4), "rounds": int(rounds),
+            "whole_table_s_at_this_rate": round(best / n * S, 2),
+            "node_updates_per_s": round(upd / best, 1), "fp64_tflops": round(tf, 3),
+            "fp64_frac_of_datasheet_peak": round(tf / FP64_PEAK_TFLOPS, 4),
+            "bound": "latency / barrier per level (DESIGN.md 7.4b), not fp64 or HBM",
             "cpu_fmm_ms_per_sensor": round(cpu * 1e3 / m, 4), "cpu_threads": os.cpu_count(), "cpu_sample_sensors": m,
-            "speedup_vs_cpu_fmm": round((cpu / m) / (best / S), 2), "max_ulp_vs_cpu_fmm": int(d.max())}
+            "speedup_vs_cpu_fmm": round((cpu / m) / (best / n), 2), "max_ulp_vs_cpu_fmm": int(d.max())}
 
 
 CONV_FLOPS_PER_UPDATE = 17      # the METHOD's arithmetic (DESIGN.md 7.4c): delay 3 sub/mul pairs folded as 2 sub + 2 mul +
@@ -406,6 +421,7 @@ def time_steps(rig, nsteps, warmup, dist=None, repeats=REPEATS):
     first region every plan has been called once (work lists built) and at least two full rotations plus
     `warmup` steps have run, whatever --warmup says, so that a short driver run (--steps 20 --warmup 5) times
     the same steady state as a long one."""
+    from paper_1501_03869_b200.sharding import max_over_ranks
     torch = rig.torch
     rig.plan_region(nsteps)                              # capture outside the timed region
     rig.run(max(warmup, 2 * rig.R))
@@ -423,9 +439,7 @@ def time_steps(rig, nsteps, warmup, dist=None, repeats=REPEATS):
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1)
         if dist is not None:
-            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+            ms = max_over_ranks(ms, dist, device="cuda")
             dist.barrier()
         regions.append(ms)
     rig.last_regions = regions
@@ -712,7 +726,9 @@ def run_ours(args):
                 "ms_per_step": mw["ms_per_step"], "gupd_s": round(mw["gupd_s"], 1),
                 "algorithmic_bytes_over_time_vs_hbm_peak": round(mw["step_hbm_frac"], 4)}
     if do_sweep:
-        eik = eikonal_probe(geom)
+        eik = [eikonal_probe(geom),
+               eikonal_probe(W.make_geometry(3), cpu_sample=32, reps=2),                 # configs[3]: 1024 sensors, 512 x 512
+               eikonal_probe(W.make_geometry(4), sample=256, cpu_sample=16, reps=1)]     # configs[4] FULL grid, one chunk
         conv = conventional_probe(geom, traces, sm_mhz=sm_max)
         exact = exact_time_probe(geom, tau, traces, peak_gbs)
         ubp = universal_bp_probe(geom, tau, traces, peak_gbs)

@@ -65,3 +65,66 @@ def test_two_rank_frame_sharding_with_gloo():
         p.join(120)
         assert p.exitcode == 0
     assert out.get("ok") is True
+
+
+def _gpu_worker(rank, world, port, out):
+    """One process per rank, each with its OWN plan (table copy) on its device and its own frames of the batch --
+    the product path, not the oracle.  With fewer devices than ranks the ranks share device 0: no kernel of one rank
+    ever waits for another rank (there is no data-path collective), so that is a valid stand-in for placement only."""
+    import torch
+    import torch.distributed as dist
+    import workloads as W
+    import paper_1501_03869_b200 as pat
+    from _cases import prod_tau
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    dev = rank % torch.cuda.device_count()
+    torch.cuda.set_device(dev)
+    geom = W.make_geometry(0)
+    tau = prod_tau(geom)
+    B = 6
+    traces = W.make_traces(geom, tau, frames=range(B))             # every rank builds the same seeded batch
+    b, e = sharding.split_frames(B, world)[rank]
+    plan = pat.Plan(geom.n, geom.h, geom.origin, geom.c_map, geom.sensors, geom.roi_index, geom.nt, geom.fs,
+                    geom.t0, max_batch=B)
+    plan.set_travel_times(tau)
+    img = torch.full((e - b, geom.npix), float("nan"), dtype=torch.float32, device="cuda:%d" % dev)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    plan.backproject(torch.from_numpy(np.ascontiguousarray(traces[b:e])).cuda(), img, e - b)
+    ev1.record()
+    torch.cuda.synchronize()
+    ms = sharding.max_over_ranks(ev0.elapsed_time(ev1), dist)      # slowest rank defines the step (gloo: CPU tensor)
+    gathered = [None] * world
+    dist.all_gather_object(gathered, (b, e, img.cpu().numpy(), ev0.elapsed_time(ev1), plan.launches()))
+    if rank == 0:
+        whole = torch.full((B, geom.npix), float("nan"), dtype=torch.float32, device="cuda:%d" % dev)
+        plan.backproject(torch.from_numpy(np.ascontiguousarray(traces)).cuda(), whole, B)
+        torch.cuda.synchronize()
+        cat = np.concatenate([g[2] for g in sorted(gathered, key=lambda g: g[0])], axis=0)
+        ref = whole.cpu().numpy()
+        # a frame's image does not depend on the batch it is in up to the fp32 order of the cross-CTA sums
+        rel = np.linalg.norm(cat - ref) / np.linalg.norm(ref)
+        out["rel"] = float(rel)
+        out["ok"] = bool(np.isfinite(cat).all()) and rel <= 1e-5 and abs(ms - max(g[3] for g in gathered)) < 1e-9 \
+            and all(g[4] >= 2 for g in gathered)
+    plan.close()
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+def test_two_ranks_run_the_product_path_on_their_own_frames():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    mgr = ctx.Manager()
+    out = mgr.dict()
+    port = _free_port()
+    procs = [ctx.Process(target=_gpu_worker, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    for p in procs:
+        p.join(300)
+        assert p.exitcode == 0
+    assert out.get("ok") is True, dict(out)
