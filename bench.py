@@ -192,14 +192,25 @@ def eikonal_probe(geom, sample=None, cpu_sample=64, reps=3):
     d = np.abs(out[:m].cpu().numpy().view(np.int32).astype(np.int64) - tau.view(np.int32).astype(np.int64))
     nodes = float(np.prod(geom.n))
     ndim = len(geom.n)
-    upd = n * nodes * rounds * (1 << ndim)                 # node updates: every pass of every round visits every node
+    visits, iters, upd = pat.pat_eikonal_last_stats()        # work counters of the last (timed) solve
+    sweeping = upd == 0                                       # PAT_EIK_ALGO=sweep: every pass visits every node
+    if sweeping:
+        upd = n * nodes * rounds * (1 << ndim)
     tf = upd * EIK_FLOPS_PER_UPDATE[ndim] / best / 1e12
+    blk = 512 if ndim == 3 else 256
+    halo = 1000 if ndim == 3 else 324
+    # HBM traffic of the block-ordered solver: per visit the block's halo'd field (fp64) + its slowness in, the block out
+    gbs = (visits * (halo + 2 * blk) * 8.0 / best / 1e9) if not sweeping else None
     return {"workload": "%d of %d sensors on the %s grid (first-order upwind, fp64)" % (n, S, "x".join(str(v) for v in geom.n)),
+            "algorithm": "level-by-level fast sweeping" if sweeping else "block-ordered fast iterative method",
             "gpu_s": round(best, 4), "gpu_ms_per_sensor": round(best * 1e3 / n, 4), "rounds": int(rounds),
             "whole_table_s_at_this_rate": round(best / n * S, 2),
-            "node_updates_per_s": round(upd / best, 1), "fp64_tflops": round(tf, 3),
-            "fp64_frac_of_datasheet_peak": round(tf / FP64_PEAK_TFLOPS, 4),
-            "bound": "latency / barrier per level (DESIGN.md 7.4b), not fp64 or HBM",
+            "block_visits_per_block": None if sweeping else round(visits / (n * math.ceil(nodes / blk)), 2),
+            "jacobi_iterations_per_visit": None if sweeping else round(iters / max(1, visits), 2),
+            "node_updates_per_node": round(upd / (n * nodes), 2),
+            "fp64_tflops": round(tf, 3), "fp64_frac_of_datasheet_peak": round(tf / FP64_PEAK_TFLOPS, 4),
+            "field_traffic_gbs": None if gbs is None else round(gbs, 1),
+            "bound": "barrier / shared-memory latency of the in-block iterations (DESIGN.md 7.4b): neither fp64 nor HBM",
             "cpu_fmm_ms_per_sensor": round(cpu * 1e3 / m, 4), "cpu_threads": os.cpu_count(), "cpu_sample_sensors": m,
             "speedup_vs_cpu_fmm": round((cpu / m) / (best / n), 2), "max_ulp_vs_cpu_fmm": int(d.max())}
 
@@ -668,7 +679,8 @@ def run_ours(args):
     geom0 = W.make_geometry(k, args.reduced)
     if args.probe:                                       # SURVEY.md 8(f) rows, off the headline path
         if args.probe == "eikonal":
-            print(json.dumps({"offline_eikonal": eikonal_probe(geom0)}))
+            print(json.dumps({"offline_eikonal": eikonal_probe(geom0, sample=1024 if k == 4 and not args.reduced else None,
+                                                               cpu_sample=16 if k == 4 else 64, reps=2)}))
         elif args.probe == "ubp":
             g1, tau1, tr1 = prepare_inputs(k, args.reduced, max(1, args.batch or 1))
             print(json.dumps({"universal_bp": universal_bp_probe(g1, tau1, tr1, peak_gbs, batches=(args.batch or 1,))}))
@@ -728,7 +740,7 @@ def run_ours(args):
     if do_sweep:
         eik = [eikonal_probe(geom),
                eikonal_probe(W.make_geometry(3), cpu_sample=32, reps=2),                 # configs[3]: 1024 sensors, 512 x 512
-               eikonal_probe(W.make_geometry(4), sample=256, cpu_sample=16, reps=1)]     # configs[4] FULL grid, one chunk
+               eikonal_probe(W.make_geometry(4), sample=1024, cpu_sample=16, reps=1)]    # configs[4] FULL grid, one chunk
         conv = conventional_probe(geom, traces, sm_mhz=sm_max)
         exact = exact_time_probe(geom, tau, traces, peak_gbs)
         ubp = universal_bp_probe(geom, tau, traces, peak_gbs)

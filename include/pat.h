@@ -303,22 +303,30 @@ pat_status pat_fmm_travel_times(const pat_grid *grid, const float *c_map,
 pat_status pat_compute_travel_times(pat_plan *plan, int32_t order, int32_t nthreads, void *stream);
 
 /* pat_eikonal_travel_times_device -- SURVEY.md 8(f) NEXT-2: the same first-order upwind system
- * solved on the GPU by sensor-batched fast sweeping (csrc/eikonal.cu): Gauss-Seidel
- * passes in the 2^ndim axis orderings, run level by level, one CTA per sensor, fp64, until a whole
- * round changes nothing.  The fixed point is what fast marching computes; rows agree with
- * pat_fmm_travel_times(order = 1) to fp32 rounding.
+ * solved on the GPU, one CTA per sensor, many sensors at once, fp64 (csrc/eikonal.cu).
+ * Default: a block-ordered fast iterative method -- the grid is cut into 8x8x8 (2-D: 16x16) blocks, the active
+ * block with the smallest arrival time on its boundary is solved next (fast marching's causal order applied to
+ * blocks) with Jacobi iterations in shared memory until nothing in it changes, and every face that changed wakes the
+ * neighbour behind it; the solve ends when no block is active.  PAT_EIK_ALGO=sweep selects round 1's level-by-level
+ * fast sweeping (also used when the grid has more blocks than one CTA's shared memory can track).  Either way the
+ * fixed point is what fast marching computes; rows agree with pat_fmm_travel_times(order = 1) to fp32 rounding.
  *   c_map, sensor_xyz, roi_index   HOST, as for pat_fmm_travel_times.
  *   tau_out      DEVICE fp32 [count][npix], written on `stream`; the call synchronises `stream`.
- *   max_rounds   cap on rounds of 2^ndim passes per sensor (<= 0: 64).
+ *   max_rounds   cap per sensor, in rounds (<= 0: 64).  A round is as much work as one visit of every block
+ *                (sweeping: 2^ndim passes over the grid); every solve takes more than one.
  *   rounds_out   HOST, may be NULL: the largest number of rounds any sensor needed.
- * Temporary device memory (one fp64 field per concurrent sensor) is allocated and freed inside.
- * A sensor outside the grid / bad c_map -> PAT_ERR_INVALID_ARG; a sensor that did not converge within
- * max_rounds -> PAT_ERR_BAD_STATE (tau_out then holds upper bounds). */
+ * Temporary device memory (one fp64 field per concurrent sensor) comes from the device-memory provider and is
+ * returned inside.  A sensor outside the grid / bad c_map -> PAT_ERR_INVALID_ARG; a sensor that did not converge
+ * within max_rounds -> PAT_ERR_BAD_STATE (tau_out then holds upper bounds). */
 pat_status pat_eikonal_travel_times_device(const pat_grid *grid, const float *c_map,
                                            const float *sensor_xyz, int32_t nsens,
                                            const int64_t *roi_index, int64_t npix,
                                            int32_t sensor_begin, int32_t count, float *tau_out,
                                            int32_t max_rounds, int32_t *rounds_out, void *stream);
+
+/* Work counters of this thread's latest pat_eikonal_travel_times_device call (block-ordered solver; zeros after a
+ * sweeping solve): blocks solved, Jacobi iterations, node updates, summed over the call's sensors.  Any pointer may be NULL. */
+pat_status pat_eikonal_last_stats(int64_t *block_visits, int64_t *jacobi_iterations, int64_t *node_updates);
 
 /* Convenience: pat_eikonal_travel_times_device on the plan's own grid / c_map / sensors, in chunks
  * through the plan's staging buffer, every row handed to pat_set_travel_times on the device. */

@@ -114,6 +114,8 @@ def lib():
                                                   ctypes.POINTER(i32), vp]
     L.pat_compute_travel_times_gpu.restype = ctypes.c_int
     L.pat_compute_travel_times_gpu.argtypes = [vp, i32, ctypes.POINTER(i32), vp]
+    L.pat_eikonal_last_stats.restype = ctypes.c_int
+    L.pat_eikonal_last_stats.argtypes = [ctypes.POINTER(i64)] * 3
     L.pat_backproject_static.restype = ctypes.c_int
     L.pat_backproject_static.argtypes = [vp, vp, vp, i32, i64, i32, i32, f32, f32, i32, vp]
     L.pat_backproject_static_max_samples.restype = i64
@@ -342,6 +344,13 @@ def pat_eikonal_travel_times_device(grid, c_map, sensor_xyz, nsens, roi_index, n
     if st != PAT_OK:
         raise PatError(st, "pat_eikonal_travel_times_device failed")
     return r.value
+
+
+def pat_eikonal_last_stats():
+    """(block visits, Jacobi iterations, node updates) of this thread's latest GPU eikonal call."""
+    v = [ctypes.c_int64(0) for _ in range(3)]
+    lib().pat_eikonal_last_stats(*[ctypes.byref(x) for x in v])
+    return tuple(int(x.value) for x in v)
 
 
 def pat_compute_travel_times_gpu(plan, max_rounds=0, stream=None):

@@ -149,3 +149,26 @@ def test_plan_compute_travel_times_gpu_end_to_end():
     # a tau that differs by an ulp can move a pixel across a sample boundary: linear interpolation is
     # continuous there, so the image moves by O(ulp) too
     assert_parity(got, ref, "gpu tau -> image")
+
+
+def test_block_ordered_solver_and_fast_sweeping_agree(monkeypatch):
+    """The default block-ordered solver and round 1's level-by-level fast sweeping (PAT_EIK_ALGO=sweep) solve the
+    same discrete system: rows within 1 ulp of each other in 2-D (ragged blocks: 70 x 45 is no multiple of 16) and 3-D,
+    and the work counters say which one ran."""
+    import paper_1501_03869_b200 as pat
+    for n, origin in [((70, 45), (0.0, 0.0)), ((21, 19, 26), (0.0, 0.0, 0.0))]:
+        h = _f32(1.0e-4)
+        rng = np.random.default_rng(11)
+        shape = tuple(reversed(n))
+        c = (1500.0 * (1.0 + 0.3 * rng.uniform(-1, 1, size=shape))).astype(np.float32)
+        hi = [(v - 1) * float(h) for v in n]
+        sens = np.zeros((3, 3), dtype=np.float32)
+        sens[:, :len(n)] = rng.uniform(0.05, 0.95, size=(3, len(n))) * np.asarray(hi)
+        monkeypatch.delenv("PAT_EIK_ALGO", raising=False)
+        a, _ = _solve_gpu(n, h, origin, c, sens, None)
+        assert pat.pat_eikonal_last_stats()[0] > 0
+        monkeypatch.setenv("PAT_EIK_ALGO", "sweep")
+        b, _ = _solve_gpu(n, h, origin, c, sens, None)
+        assert pat.pat_eikonal_last_stats() == (0, 0, 0)
+        monkeypatch.delenv("PAT_EIK_ALGO", raising=False)
+        assert np.isfinite(a).all() and _ulp_diff(a, b).max() <= 1

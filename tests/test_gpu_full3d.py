@@ -44,7 +44,7 @@ def test_config4_full_size_sampled_voxels():
     tau_abs = np.empty((S, apos.size), np.float32)
     check_sensors = sorted(set(int(v) for v in rng.integers(0, S, size=8)) | {0, S - 1})
     tau_check = {}
-    chunk = 256
+    chunk = 1024
     rows = torch.empty((chunk, P), dtype=torch.float32, device="cuda")
     t_eik, rounds = time.time(), 0
     for s0 in range(0, S, chunk):
