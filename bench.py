@@ -474,22 +474,26 @@ def kernel_only_ms(rig, mode, nsteps, warmup):
     return ms / nsteps
 
 
-def host_enqueue_us(rig, n=300):
+def host_enqueue_us(rig, burst=64, bursts=15):
     """Host wall-clock microseconds one direct pat_backproject call takes to ENQUEUE (ctypes marshalling
-    included), the GPU idle at the start and never waited for inside the loop."""
+    included).  Measured in short bursts that start on an idle GPU: a long loop of direct calls is throttled by
+    the GPU itself once the launch queue is full (a direct-call step takes ~12 us of GPU time) and then measures
+    the step, not the host.  Median over the bursts."""
     torch = rig.torch
     if not rig.primed:
         rig.prime()
+    out = []
     with torch.cuda.stream(rig.stream):
         for i in range(rig.R):
             rig.step(i)
-        torch.cuda.synchronize()
-        t = time.perf_counter()
-        for i in range(n):
-            rig.step(i)
-        dt = time.perf_counter() - t
+        for _ in range(bursts):
+            torch.cuda.synchronize()
+            t = time.perf_counter()
+            for i in range(burst):
+                rig.step(i)
+            out.append((time.perf_counter() - t) / burst * 1e6)
     torch.cuda.synchronize()
-    return dt / n * 1e6
+    return float(np.median(out))
 
 
 def measure(geom, tau, traces, B, steps, warmup, variant, dist, peak_gbs, sm_mhz, do_e2e, kernels=True,
