@@ -467,12 +467,15 @@ pat_status ensure_onfly(pat_plan *p, float c0, float c0_hi, void *stream, PatOnf
         const int64_t nrows = p->dims.ntiles * S;
         // scratch for the row ranges: the workspace's meta array is the table path's; same size, own block
         PatDevBuf mbuf;
-        if (!plan_alloc(p, (size_t)nrows * 8, &mbuf))
+        if (!plan_alloc(p, (size_t)nrows * 8 + 256, &mbuf))
             return fail(p, PAT_ERR_NOMEM, "conventional BP row ranges: the device-memory provider returned nothing");
         void *d_meta = mbuf.p;
-        cudaError_t e = cudaSuccess;
+        int32_t *d_bad = (int32_t *)((char *)mbuf.p + (size_t)nrows * 8);        // any |r - s|^2 outside the fast range?
+        cudaError_t e = cudaMemsetAsync(d_bad, 0, sizeof(int32_t), st);
         PatLaunchCtx ctx{stream, p->num_sms, false};
-        int le = pat_launch_onfly_meta(ctx, *out, S, d_meta, nrows, p->dims.nt);
+        int le = e == cudaSuccess ? pat_launch_onfly_meta(ctx, *out, S, d_meta, nrows, p->dims.nt, d_bad) : (int)e;
+        int32_t bad = 1;
+        if (!le) e = cudaMemcpyAsync(&bad, d_bad, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
         ++p->launches;
         try { p->onfly_meta.resize((size_t)nrows * 2); } catch (...) { cudaStreamSynchronize(st); plan_free(p, &mbuf); return fail(p, PAT_ERR_NOMEM, "host allocation failed"); }
         if (!le) e = cudaMemcpyAsync(p->onfly_meta.data(), d_meta, (size_t)nrows * 8, cudaMemcpyDeviceToHost, st);
@@ -517,6 +520,7 @@ pat_status ensure_onfly(pat_plan *p, float c0, float c0_hi, void *stream, PatOnf
         if (le || e != cudaSuccess) { p->onfly_meta.clear(); return cuda_fail(p, le ? le : (int)e, "conventional BP row ranges"); }
         p->onfly_c0 = c0;
         p->onfly_c0_hi = c0_hi;
+        p->onfly_d2_in_range = bad == 0;
         needed_samples(p->onfly_meta, p->dims.nt, &p->onfly_lo, &p->onfly_hi);
         // work lists of the previous c0 are stale
         for (size_t q = 0; q < p->schedules.size();) {
@@ -528,6 +532,8 @@ pat_status ensure_onfly(pat_plan *p, float c0, float c0_hi, void *stream, PatOnf
             }
         }
     }
+    // the gather may use the written-out square root and skip "- t0" (gather.cu, onfly_u_fast2d): bit-identical there
+    out->fast2d = p->grid.ndim == 2 && p->t0 == 0.0f && p->onfly_d2_in_range && !p->env.no_fast_delays;
     return PAT_OK;
 }
 
@@ -628,6 +634,7 @@ extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, cons
         p->env.slow_cost = std::max(1, env_int("PAT_SLOW_COST", 5));
         p->env.debug = env_int("PAT_DEBUG", 0) == 1;
         p->env.chain_depth = env_int("PAT_CHAIN_DEPTH", 3);
+        p->env.no_fast_delays = env_int("PAT_NO_FAST_DELAYS", 0) == 1;   // A/B: the generic delay arithmetic in the conventional BP
         if (const char *fn = std::getenv("PAT_SCHED_DUMP")) p->env.sched_dump = fn;
     }
     env = std::getenv("PAT_TRACE_FILE");                   // diagnostic: per-CTA timeline of the last gather launch

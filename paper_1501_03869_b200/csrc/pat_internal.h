@@ -63,6 +63,7 @@ struct PatTune {
     int chunk_cost = 6, slow_cost = 5;
     bool debug = false;
     int chain_depth = 3;          // PAT_CHAIN_DEPTH (A/B): 3 = the pre-pass of call j hangs on the gather of call j-3, 2 = on j-2
+    bool no_fast_delays = false;  // PAT_NO_FAST_DELAYS=1 (A/B): conventional BP always with the generic delay arithmetic
     std::string sched_dump;
 };
 
@@ -74,6 +75,7 @@ struct PatOnfly {
     float inv_c0 = 0, t0 = 0, fs = 0;
     int32_t ndim = 2;
     int32_t nsweep = 0;                 // > 0: pat_backproject_conventional_sweep, one image per speed
+    bool fast2d = false;                // 2-D, t0 = 0, every |r - s|^2 in [1e-30, 1e30]: the gather may use onfly_u_fast2d
     float sweep_inv_c0[PAT_MAX_SWEEP] = {};
 };
 
@@ -147,6 +149,7 @@ struct pat_plan {
     // conventional BP (pat_backproject_conventional): geometry on the device, k-ranges for the current c0
     std::vector<int32_t> host_perm;   // tile slot -> ROI position (-1 = padding)
     float *d_pix = nullptr, *d_sens = nullptr;
+    bool onfly_d2_in_range = false;         // every |r - s|^2 of the plan is inside [1e-30, 1e30] (onfly_meta_kernel)
     float onfly_c0 = 0, onfly_c0_hi = 0;   // speed (range, for a sweep) the row ranges below were computed for
     std::vector<int32_t> onfly_meta;
     // pat_set_pixel_weights / pat_compute_solid_angle_weights: per-(sensor, pixel) factors, tile-major like u_t
@@ -217,6 +220,7 @@ int pat_launch_fill(const PatLaunchCtx &ctx, float *dst, int64_t n, float value)
 // [3][slots] node coordinates per tile slot, sens / nrm = float [nsens][3] (all device).
 int pat_launch_solid_angle(const PatLaunchCtx &ctx, const double *pix, int64_t slots, const float *sens,
                            const float *nrm, int32_t nsens, int32_t ndim, float *w_t);
-int pat_launch_onfly_meta(const PatLaunchCtx &ctx, const PatOnfly &o, int32_t nsens, void *meta, int64_t nrows, int32_t nt);
+int pat_launch_onfly_meta(const PatLaunchCtx &ctx, const PatOnfly &o, int32_t nsens, void *meta, int64_t nrows, int32_t nt,
+                          int32_t *d2_out_of_range = nullptr);
 
 #endif  // PAT_INTERNAL_H_

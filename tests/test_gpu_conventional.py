@@ -194,3 +194,50 @@ def test_c0_sweep_with_speeds_that_push_delays_out_of_the_record_and_argument_er
             assert ei.value.status == pat.PAT_ERR_INVALID_ARG
     finally:
         plan.close()
+
+
+def test_fast_delays_are_the_generic_delays_and_a_detector_on_a_node_switches_them_off(monkeypatch):
+    """The one-frame conventional BP computes 2-D, t0 = 0 delays with the square root written out (gather.cu,
+    onfly_u_fast2d): valid only while every |r - s|^2 is a normal number, which the set-up kernel checks per plan.
+    (a) default (fast) and PAT_NO_FAST_DELAYS=1 (generic) both match the oracle on configs[0] -- the image moves
+    by rel-L2 ~1e-5 if a single rounding of the delay differs (gather.cu, note on packed multiplies); (b) with one
+    detector moved ONTO a node |r - s| = 0 occurs (rsqrt(0) = inf: the fast path would produce NaN -> a dropped term;
+    the oracle's sqrt gives 0 -> u = 0, a valid term), the plan must fall back and still match; (c) the c0 sweep too."""
+    import torch
+    geom = W.make_geometry(0)
+    c0 = 1560.0
+    rng = np.random.default_rng(41)
+    traces = rng.standard_normal((1, geom.nsens, geom.nt)).astype(np.float32)
+    traces[:, :, :3] += 5.0                                        # make the u = 0 term of (b) count
+    c0s = np.array([1500.0, 1560.0, 1610.0], dtype=np.float32)
+
+    def check(sensors, tag):
+        g = W.make_geometry(0)
+        g.sensors = sensors
+        tau = oracle.tau_conventional(g.n, g.h, g.origin, sensors, g.roi_index, c0)
+        ref = oracle.backproject(tau, traces, g.fs, g.t0, 1)
+        plan = _plan(g, 1)
+        try:
+            assert_parity(_run(plan, traces, c0, g.npix), ref, tag)
+            img = torch.full((len(c0s), g.npix), float("nan"), dtype=torch.float32, device="cuda")
+            plan.backproject_conventional_sweep(torch.from_numpy(traces[0]).cuda(), img, c0s)
+            torch.cuda.synchronize()
+            for q, c in enumerate(c0s):
+                tq = oracle.tau_conventional(g.n, g.h, g.origin, sensors, g.roi_index, float(c))
+                assert_parity(img[q:q + 1].cpu().numpy(), oracle.backproject(tq, traces, g.fs, g.t0, 1), tag + " sweep c0=%g" % c)
+        finally:
+            plan.close()
+        return tau
+
+    check(geom.sensors.copy(), "fast delays")
+    monkeypatch.setenv("PAT_NO_FAST_DELAYS", "1")
+    check(geom.sensors.copy(), "generic delays")
+    monkeypatch.delenv("PAT_NO_FAST_DELAYS")
+    on_node = geom.sensors.copy()
+    j = geom.npix // 2 + 5                                        # node (i, j) of the 64 x 64 grid: its fp32 coordinates
+    q = int(geom.roi_index[j])
+    ix, iy = q % geom.n[0], q // geom.n[0]
+    on_node[3, 0] = np.float32(geom.origin[0]) + np.float32(ix) * np.float32(geom.h)
+    on_node[3, 1] = np.float32(geom.origin[1]) + np.float32(iy) * np.float32(geom.h)
+    tau = check(on_node, "a detector on a node")
+    assert tau[3, j] == 0.0
