@@ -424,6 +424,9 @@ pat_status get_schedule(pat_plan *p, int bp, bool onfly, PatSchedule **out) {
     } timer{p, t_begin};
     PatGatherConfig cfg = pat_gather_config(bp, p->tune_wr, p->tune_R, p->tune_stages, onfly, p->exact,
                                             p->d_w_t != nullptr, p->env);
+    // the occupancy the work list is cut for is that of the kernel that will run (ensure_onfly came first)
+    cfg.fastu = onfly && bp == 1 && !p->exact && !p->d_w_t && p->grid.ndim == 2 && p->t0 == 0.0f &&
+                p->onfly_d2_in_range && !p->env.no_fast_delays;
     return build_schedule(p, cfg, out);
 }
 

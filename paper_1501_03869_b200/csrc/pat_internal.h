@@ -53,6 +53,7 @@ struct PatGatherConfig {
     bool onfly = false;       // work list of the conventional BP (k-ranges from the geometry, no table)
     bool exact = false;       // PAT_W_*_EXACT: the bp "frames" are channel pairs {wp*p, -wd*D} of bp/2 frames
     bool weighted = false;    // pat_set_pixel_weights: a stage holds R weight rows after its R u rows
+    bool fastu = false;       // conventional BP, one frame, fast delays (gather.cu onfly_u_fast2d): its own instantiation
 };
 
 // Tuning / diagnostic knobs, read from the environment ONCE, in pat_plan_create (never on a call path):
