@@ -149,7 +149,10 @@ pat_status pat_set_travel_times(pat_plan *plan, const float *tau, int32_t sensor
  * builds that class's work list on the host (memory from the device-memory provider, size under "device memory"
  * above: 0.7 MB for configs[1], ~0.6 GB and 0.7 s for the 34 GB table of configs[4]) and uploads it synchronously;
  * that first call must therefore not happen inside a stream capture.
- * A plan is driven from ONE stream at a time; traces and images must not overlap.
+ * A plan is driven from ONE stream at a time, with the device it was created on current (another current device ->
+ * PAT_ERR_INVALID_ARG); traces and images must not overlap.  HOST traces must be complete in memory when the call is
+ * made: their copy runs on the plan's own copy stream and is NOT ordered behind work already enqueued on `stream`
+ * (a pinned buffer still being filled by an earlier stream-ordered copy or callback would be read too early).
  * Consecutive calls (cross-call overlap).  Inside a stream capture -- the way to run a ~10 us frame without paying
  * a launch gap per kernel -- consecutive calls with DEVICE buffers are captured with explicit graph edges instead of
  * a linear chain: the gather of call j hangs on the gather of call j-1 by a programmatic edge (its CTAs take over

@@ -414,6 +414,17 @@ pat_status build_schedule(pat_plan *p, const PatGatherConfig &cfg, PatSchedule *
     return PAT_OK;
 }
 
+// Every device-side call of a plan must run with the plan's device current: its workspace, work lists and streams
+// belong to it, and memory from the provider would otherwise come from another device.
+pat_status check_device(pat_plan *p) {
+    int cur = -1;
+    cudaError_t e = cudaGetDevice(&cur);
+    if (e != cudaSuccess) return cuda_fail(p, e, "cudaGetDevice");
+    if (cur != p->device)
+        return fail(p, PAT_ERR_INVALID_ARG, "the current CUDA device is not the one the plan was created on (cudaSetDevice first)");
+    return PAT_OK;
+}
+
 pat_status get_schedule(pat_plan *p, int bp, bool onfly, PatSchedule **out) {
     for (PatSchedule &sc : p->schedules)
         if (sc.cfg.bp == bp && sc.cfg.onfly == onfly) { *out = &sc; return PAT_OK; }
@@ -754,6 +765,7 @@ static pat_status upload_rows(pat_plan *p, const float *src, int32_t sensor_begi
 extern "C" pat_status pat_set_travel_times(pat_plan *p, const float *tau, int32_t sensor_begin,
                                            int32_t count, void *stream) {
     if (!p) return PAT_ERR_INVALID_ARG;
+    if (pat_status ds = check_device(p)) return ds;
     if (!tau && count > 0) return fail(p, PAT_ERR_INVALID_ARG, "tau is NULL");
     if (sensor_begin < 0 || count < 0 || sensor_begin > p->dims.nsens - count)
         return fail(p, PAT_ERR_INVALID_ARG, "sensor range outside [0, nsens)");
@@ -779,6 +791,7 @@ extern "C" pat_status pat_backproject(pat_plan *p, const float *traces, float *i
 extern "C" pat_status pat_backproject_conventional(pat_plan *p, const float *traces, float *images,
                                                    int32_t nframes, float c0, void *stream) {
     if (!p) return PAT_ERR_INVALID_ARG;
+    if (pat_status ds = check_device(p)) return ds;
     if (!(c0 > 0.0f) || !std::isfinite(c0)) return fail(p, PAT_ERR_INVALID_ARG, "c0 must be finite and > 0");
     if (p->sensors.empty()) return fail(p, PAT_ERR_BAD_STATE, "plan was created without sensor_xyz");
     return backproject_impl(p, traces, images, nframes, stream, true, c0);
@@ -1092,6 +1105,7 @@ extern "C" pat_status pat_compute_travel_times(pat_plan *p, int32_t order, int32
 extern "C" pat_status pat_compute_travel_times_gpu(pat_plan *p, int32_t max_rounds, int32_t *rounds_out,
                                                    void *stream) {
     if (!p) return PAT_ERR_INVALID_ARG;
+    if (pat_status ds = check_device(p)) return ds;
     if (p->c_map.empty() || p->sensors.empty())
         return fail(p, PAT_ERR_BAD_STATE, "plan was created without c_map / sensor_xyz");
     float *stage = (float *)(p->ws + p->lay.tau_stage);
@@ -1135,6 +1149,7 @@ static pat_status ensure_weight_table(pat_plan *p, void *stream) {
 extern "C" pat_status pat_set_pixel_weights(pat_plan *p, const float *w, int32_t sensor_begin, int32_t count,
                                             void *stream) {
     if (!p) return PAT_ERR_INVALID_ARG;
+    if (pat_status ds = check_device(p)) return ds;
     if (!w) {                                           // remove the weights
         if (count != 0) return fail(p, PAT_ERR_INVALID_ARG, "w is NULL");
         if (p->d_w_t) {
@@ -1155,6 +1170,7 @@ extern "C" pat_status pat_set_pixel_weights(pat_plan *p, const float *w, int32_t
 
 extern "C" pat_status pat_compute_solid_angle_weights(pat_plan *p, const float *normals, void *stream) {
     if (!p) return PAT_ERR_INVALID_ARG;
+    if (pat_status ds = check_device(p)) return ds;
     if (!normals) return fail(p, PAT_ERR_INVALID_ARG, "normals is NULL");
     if (p->sensors.empty()) return fail(p, PAT_ERR_BAD_STATE, "plan was created without sensor_xyz");
     const int32_t S = p->dims.nsens;
@@ -1202,6 +1218,7 @@ extern "C" pat_status pat_compute_solid_angle_weights(pat_plan *p, const float *
 
 extern "C" pat_status pat_set_roi_mask(pat_plan *p, const uint8_t *mask) {
     if (!p) return PAT_ERR_INVALID_ARG;
+    if (pat_status ds = check_device(p)) return ds;
     cudaError_t e = cudaDeviceSynchronize();            // no launch may still read the old permutation / lists
     if (e != cudaSuccess) return cuda_fail(p, e, "synchronise");
     drop_schedules(p);
