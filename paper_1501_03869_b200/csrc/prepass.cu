@@ -10,6 +10,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cstdlib>
 
 namespace {
 
@@ -221,6 +222,61 @@ prepass_blocked_kernel(const float *__restrict__ traces, float *__restrict__ b, 
     prepass_block_done(ready);
 }
 
+constexpr int kB1Threads = 128, kB1U = 4;            // block size and quads per thread of the kernels written to run beside gathers
+
+// The same for 16-byte aligned rows (nt % 4 == 0), written to run BESIDE running gathers like prepass_b1_kernel: the
+// (frame slot, sensor, quad) items are one flat index space -- the kernel above spends a 256-thread block on the 136
+// quads of one (frame, sensor) row of configs[1], 2048 of them at B = 4, and runs 2 - 3 blocks per SM beside three
+// resident gather CTAs: 5 - 7 waves of a load -> store round trip each -- small blocks (128 threads, <= 64 registers),
+// kB1U quads per thread a quarter of the grid apart, all loads issued before any is used.
+__global__ void __launch_bounds__(kB1Threads, 8)
+prepass_blocked_flat_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
+                            int32_t nsens, int32_t nt, int32_t ntb, int32_t nframes, int32_t log2_bp, int64_t nzero,
+                            float wp, float wd, float t0fs, int32_t n_lo, int32_t quads, uint32_t total, uint32_t *ready) {
+    asm volatile("griddepcontrol.launch_dependents;");
+    const uint32_t gid = blockIdx.x * kB1Threads + threadIdx.x, nthr = gridDim.x * kB1Threads;
+    for (uint32_t q = gid; q < (uint32_t)nzero; q += nthr) images[q] = 0.0f;
+    const uint32_t per_frame = (uint32_t)nsens * (uint32_t)quads, bpm = (1u << log2_bp) - 1u;
+    for (uint32_t q = gid; q < total; q += kB1U * nthr) {
+        float w[kB1U][6];
+        uint32_t f[kB1U], srow[kB1U];
+        int32_t n0[kB1U];
+#pragma unroll
+        for (int u = 0; u < kB1U; ++u) {
+            const uint32_t qq = min(q + u * nthr, total - 1u);                   // past the end: redo the last quad (harmless)
+            f[u] = qq / per_frame;
+            const uint32_t r = qq - f[u] * per_frame;
+            srow[u] = r / (uint32_t)quads;
+            n0[u] = n_lo + (int32_t)((r - srow[u] * (uint32_t)quads) << 2);
+#pragma unroll
+            for (int j = 0; j < 6; ++j) w[u][j] = 0.0f;
+            if (f[u] < (uint32_t)nframes && n0[u] < nt) {                        // padding frames of the group, samples past the record: zeros
+                const float *p = traces + ((size_t)f[u] * nsens + srow[u]) * nt + n0[u];
+                const float4 v = __ldg(reinterpret_cast<const float4 *>(p));
+                w[u][0] = n0[u] > 0 ? __ldg(p - 1) : 0.0f;
+                w[u][5] = n0[u] + 4 < nt ? __ldg(p + 4) : 0.0f;
+                w[u][1] = v.x; w[u][2] = v.y; w[u][3] = v.z; w[u][4] = v.w;
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < kB1U; ++u) {
+            float4 o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            if (f[u] < (uint32_t)nframes && n0[u] < nt) {
+                if (quad_interior(n0[u], nt, wd)) {
+                    o = weight_quad_interior(w[u], n0[u], wp, t0fs);
+                } else {
+                    o.x = weight_at(w[u] + 0, n0[u] + 0, nt, wp, wd, t0fs); o.y = weight_at(w[u] + 1, n0[u] + 1, nt, wp, wd, t0fs);
+                    o.z = weight_at(w[u] + 2, n0[u] + 2, nt, wp, wd, t0fs); o.w = weight_at(w[u] + 3, n0[u] + 3, nt, wp, wd, t0fs);
+                }
+            }
+            const uint32_t g = f[u] >> log2_bp, fl = f[u] & bpm;
+            float *dst = b + ((((size_t)g * nsens + srow[u]) * ntb + (uint32_t)(n0[u] >> 5)) << log2_bp) * 32 + (size_t)fl * 32 + (n0[u] & 31);
+            *reinterpret_cast<float4 *>(dst) = o;
+        }
+    }
+    prepass_block_done(ready);
+}
+
 // Bp = 16 (interleaved [sensor][sample][16], gather.cu PPL == 4).
 __global__ void __launch_bounds__(256)
 prepass_il16_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
@@ -280,7 +336,6 @@ prepass_il16_kernel(const float *__restrict__ traces, float *__restrict__ b, flo
 // remainder -- 128 threads x <= 64 registers -- whose threads take kB1U quads a quarter of the grid apart and issue
 // all their loads before they use any (a 256-thread block of 40 registers is an exact fit on paper and was not
 // co-scheduled: its blocks only started when gather CTAs left; one quad per thread needed two waves).
-constexpr int kB1Threads = 128, kB1U = 4;
 __global__ void __launch_bounds__(kB1Threads, 8)
 prepass_b1_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
                   int32_t nsens, int32_t nt, int32_t nt4, int64_t nzero, float wp, float wd, float t0fs,
@@ -568,6 +623,16 @@ int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, f
                               nframes, npix, wp, wd, t0fs, n_lo, quads, ready, ctx.pre_trace);
         return launch_pre(ctx, prepass_small_kernel<2>, dim3((unsigned)blocks), 256, traces, b, images, nsens, nt, nt4,
                           nframes, npix, wp, wd, t0fs, n_lo, quads, ready, ctx.pre_trace);
+    }
+    if (blocked && (nt & 3) == 0 && std::getenv("PAT_OLD_BLOCKED_PREPASS") == nullptr) {
+        const int32_t groups = (nframes + bp - 1) / bp;
+        const int64_t total = (int64_t)groups * bp * nsens * quads;
+        if (total < (1ll << 31) && nzero < (1ll << 32)) {
+            int64_t nb = (total + kB1Threads * kB1U - 1) / (kB1Threads * kB1U);
+            if (nb > (int64_t)ctx.num_sms * 8) nb = (int64_t)ctx.num_sms * 8;
+            return launch_pre(ctx, prepass_blocked_flat_kernel, dim3((unsigned)std::max<int64_t>(nb, 1)), kB1Threads, traces, b, images,
+                              nsens, nt, ntb, nframes, log2_bp, nzero, wp, wd, t0fs, n_lo, quads, (uint32_t)total, ready);
+        }
     }
     if (blocked) {
         const int32_t groups = (nframes + bp - 1) / bp;
