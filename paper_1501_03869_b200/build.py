@@ -27,7 +27,7 @@ def build(force: bool = False, verbose: bool = False, trace: bool = False) -> st
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
-    extra = os.environ.get("PAT_NVCC_FLAGS", "").split()          # experiments: e.g. PAT_NVCC_FLAGS=-DPAT_IL48=1
+    extra = os.environ.get("PAT_NVCC_FLAGS", "").split()          # experiments: e.g. PAT_NVCC_FLAGS=-DPAT_LEGACY_LAYOUTS=1
     cmd = [NVCC, *FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), *(["-DPAT_TRACE_BUILD"] if trace else []),
            "-o", tmp, *srcs, "-lgomp"]
     subprocess.run(cmd, check=True)
