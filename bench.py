@@ -474,11 +474,12 @@ def kernel_only_ms(rig, mode, nsteps, warmup):
     return ms / nsteps
 
 
-def host_enqueue_us(rig, burst=64, bursts=15):
+def host_enqueue_us(rig, burst=64, bursts=60):
     """Host wall-clock microseconds one direct pat_backproject call takes to ENQUEUE (ctypes marshalling
     included).  Measured in short bursts that start on an idle GPU: a long loop of direct calls is throttled by
     the GPU itself once the launch queue is full (a direct-call step takes ~12 us of GPU time) and then measures
-    the step, not the host.  Median over the bursts."""
+    the step, not the host.  Median over the last third of the bursts: the first ones run on a host core that has been
+    idling in synchronize calls and has not clocked up yet (13.7 us per call falling to 7.5 us on the same box)."""
     torch = rig.torch
     if not rig.primed:
         rig.prime()
@@ -493,7 +494,8 @@ def host_enqueue_us(rig, burst=64, bursts=15):
                 rig.step(i)
             out.append((time.perf_counter() - t) / burst * 1e6)
     torch.cuda.synchronize()
-    return float(np.median(out))
+    rig.enqueue_bursts_us = [round(v, 2) for v in out]
+    return float(np.median(out[-(bursts // 3):]))
 
 
 def measure(geom, tau, traces, B, steps, warmup, variant, dist, peak_gbs, sm_mhz, do_e2e, kernels=True,
@@ -528,6 +530,7 @@ def measure(geom, tau, traces, B, steps, warmup, variant, dist, peak_gbs, sm_mhz
         smem_upd_s = SMEM_BYTES_PER_CLK_SM / 8.0 * sms * sm_mhz * 1e6
         out["sm_side_frac"] = (upd / (gat_ms * 1e-3)) / smem_upd_s
         out["host_enqueue_us"] = host_enqueue_us(rig)
+        out["host_enqueue_bursts_us"] = rig.enqueue_bursts_us
     out["launches_per_step"] = rig.plans[0].launches_per_call() if hasattr(rig.plans[0], "launches_per_call") else 2
     out["direct_call_launches_seen"] = rig.launches() - l0
     rig.close()
@@ -773,7 +776,8 @@ def run_ours(args):
                     "timing": "median of %d regions of exactly `steps` steps each (CUDA events on the launching "
                               "stream, max over ranks per region), after >= 2 full plan rotations of warm-up" % REPEATS,
                     "regions_ms_per_step": main["regions_ms_per_step"],
-                    "host_enqueue_us_per_direct_call": round(main["host_enqueue_us"], 2)},
+                    "host_enqueue_us_per_direct_call": round(main["host_enqueue_us"], 2),
+                    "host_enqueue_bursts_us": main["host_enqueue_bursts_us"]},
         "host_enqueue_us": round(main["host_enqueue_us"], 2),
         "gpu_launches": int(main["launches_per_step"] * args.steps),
         "clocks": clocks_main,
