@@ -648,6 +648,7 @@ extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, cons
         p->env.slow_cost = std::max(1, env_int("PAT_SLOW_COST", 5));
         p->env.debug = env_int("PAT_DEBUG", 0) == 1;
         p->env.chain_depth = env_int("PAT_CHAIN_DEPTH", 3);
+        p->env.old_blocked_prepass = env_int("PAT_OLD_BLOCKED_PREPASS", 0) == 1;
         p->env.no_fast_delays = env_int("PAT_NO_FAST_DELAYS", 0) == 1;   // A/B: the generic delay arithmetic in the conventional BP
         if (const char *fn = std::getenv("PAT_SCHED_DUMP")) p->env.sched_dump = fn;
     }
@@ -953,6 +954,7 @@ static pat_status backproject_impl(pat_plan *p, const float *traces, float *imag
     const bool prof = p->profiling == 1 && p->prof_events.size() < 3u * 65536u;
     PatLaunchCtx ctx{stream, p->num_sms, p->use_pdl && !prof};
     ctx.high_priority = p->prio_high;
+    ctx.old_blocked_prepass = p->env.old_blocked_prepass;
     const size_t ibytes = (size_t)nimages * d.npix * sizeof(float);
     const bool do_gather = sc->grid_x > 0 && p->profiling != 3;
     const bool do_pre = p->profiling != 2;

@@ -64,6 +64,7 @@ struct PatTune {
     int chunk_cost = 6, slow_cost = 5;
     bool debug = false;
     int chain_depth = 3;          // PAT_CHAIN_DEPTH (A/B): 3 = the pre-pass of call j hangs on the gather of call j-3, 2 = on j-2
+    bool old_blocked_prepass = false;   // PAT_OLD_BLOCKED_PREPASS=1 (A/B)
     bool no_fast_delays = false;  // PAT_NO_FAST_DELAYS=1 (A/B): conventional BP always with the generic delay arithmetic
     std::string sched_dump;
 };
@@ -170,6 +171,7 @@ struct PatLaunchCtx {
     bool use_pdl;
     unsigned long long *pre_trace = nullptr;   // PAT_TRACE_FILE diagnostic: {pre-pass block 0 start, flag raised}
     int high_priority = 0;                     // the device's greatest stream priority (pre-pass launches)
+    bool old_blocked_prepass = false;          // PAT_OLD_BLOCKED_PREPASS=1 at plan creation (A/B): round 1's blocked pre-pass kernel
 };
 
 // tau rows [sensor_begin, +count) from src[count][npix] (device) -> u_t (tile-major, u = (tau-t0)*fs).

@@ -624,7 +624,7 @@ int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, f
         return launch_pre(ctx, prepass_small_kernel<2>, dim3((unsigned)blocks), 256, traces, b, images, nsens, nt, nt4,
                           nframes, npix, wp, wd, t0fs, n_lo, quads, ready, ctx.pre_trace);
     }
-    if (blocked && (nt & 3) == 0 && std::getenv("PAT_OLD_BLOCKED_PREPASS") == nullptr) {
+    if (blocked && (nt & 3) == 0 && !ctx.old_blocked_prepass) {
         const int32_t groups = (nframes + bp - 1) / bp;
         const int64_t total = (int64_t)groups * bp * nsens * quads;
         if (total < (1ll << 31) && nzero < (1ll << 32)) {

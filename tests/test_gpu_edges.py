@@ -349,3 +349,17 @@ def test_back_to_back_single_frame_calls_on_one_plan():
             assert_parity(outs[q].cpu().numpy(), ref, "back-to-back call %d" % q)
     finally:
         plan.close()
+
+
+@pytest.mark.parametrize("env", ["PAT_PLAIN_MORTON", "PAT_OLD_BLOCKED_PREPASS"])
+@pytest.mark.parametrize("B", [1, 4, 16])
+def test_ab_switches_of_the_layout_give_the_same_images(monkeypatch, env, B):
+    """The pixel order (recursive bisection vs round 1's plain Morton order) and the two pre-pass kernels of the
+    blocked layout are implementation choices: the oracle does not know them, so both settings must meet the bar
+    (configs[1]: a disk that cuts Morton blocks -- the case the bisection order exists for)."""
+    geom, tau = case(1)
+    traces = W.make_traces(geom, tau, frames=range(20, 20 + B))
+    ref = oracle.backproject(tau, traces, geom.fs, geom.t0, 1)
+    assert_parity(gpu_backproject(geom, tau, traces), ref, "default B=%d" % B)
+    monkeypatch.setenv(env, "1")                         # read when the plan is created
+    assert_parity(gpu_backproject(geom, tau, traces), ref, "%s=1 B=%d" % (env, B))
