@@ -14,8 +14,8 @@ CPU FMM (input preparation, untimed).  Prints ONE JSON line (rank 0):
                is called once and two full rotations run before the first region, whatever --warmup is.
   roofline     the gather kernel alone: algorithmic bytes per launch (tau + traces + images,
                north_star's definition) / its mean launch duration (the gather launched back to back
-               from the same kind of CUDA graph, pat_set_profiling mode 2, CUDA events around the
-               region), against the measured HBM copy peak of MEASURED_PEAKS.json.
+               from the same kind of CUDA graph, pat_set_profiling mode 2, CUDA events around regions of
+               >= 240 launches whatever --steps is), against the measured HBM copy peak of MEASURED_PEAKS.json.
   e2e          the same metric through the C-ABI with pinned HOST traces/images (H2D + D2H timed).
   cpu_baseline the oracle (oracle/pat_oracle.c) timed on this box's host cores, rank 0, N = 1.
   warm_l2      (labelled, not the headline) ONE plan, the same table every step -- the paper's "off-line once" case.
@@ -517,7 +517,9 @@ def measure(geom, tau, traces, B, steps, warmup, variant, dist, peak_gbs, sm_mhz
         "l2_bytes": rig.l2_bytes,
     }
     if kernels:
-        nk = max(2 * rig.R, min(steps, 1000))
+        # the kernel-only figures are their own measurement (not the K-step region): regions of >= 240 launches whatever
+        # --steps is, so that the driver's short run reports the same steady state as a long one
+        nk = max(2 * rig.R, 240, min(steps, 1000))
         gat_ms = kernel_only_ms(rig, 2, nk, min(warmup, 20))
         pre_ms = kernel_only_ms(rig, 3, nk, min(warmup, 20))
         # context for the roofline fraction: ONE kernel that only streams the step's footprint (table + b in,
@@ -716,7 +718,7 @@ def run_ours(args):
             if b == B:
                 m = main
             else:
-                st = max(20, min(args.steps, int(args.steps * 4 / b)))
+                st = max(240 // min(b, 8), min(args.steps, int(args.steps * 4 / b)))      # side rows: >= 240 frames per region
                 m = measure(geom, tau, traces, b, st, min(args.warmup, 10), tuning_of(args), None, peak_gbs,
                             sm_max, False)
             sweep.append({"B": b, "ms_per_frame": round(m["ms_per_frame"], 6),
@@ -729,7 +731,7 @@ def run_ours(args):
         # the same kernels on a table 11x larger (configs[4] reduced: 64^3 voxels x 512 sensors, 537 MB):
         # launch, prologue and tail weigh less there, so this shows the steady-state rate of the gather
         g4, tau4, tr4 = prepare_inputs(4, True, 1)
-        m4 = measure(g4, tau4, tr4, 1, max(20, args.steps // 10), min(args.warmup, 10), tuning_of(args), None,
+        m4 = measure(g4, tau4, tr4, 1, max(60, args.steps // 10), min(args.warmup, 10), tuning_of(args), None,
                      peak_gbs, sm_max, False)
         probe = {"workload": "configs[4] reduced: %d sensors x %d voxels, Nt=%d, 1 frame/step" % (g4.nsens, g4.npix, g4.nt),
                  "ms_per_frame": round(m4["ms_per_frame"], 6), "gupd_s": round(m4["gupd_s"], 1),
@@ -739,7 +741,7 @@ def run_ours(args):
     if world == 1 and k in (1, 2) and not args.no_warm:
         # the paper's use case: ONE table, computed "off-line ... once", every frame -- 43.7 MB fits
         # the L2, so consecutive steps may find it there.  Labelled; NOT the headline (which rotates plans).
-        mw = measure(geom, tau, traces, B, max(20, min(args.steps, 1000)), min(args.warmup, 10), tuning_of(args), None,
+        mw = measure(geom, tau, traces, B, max(240, min(args.steps, 1000)), min(args.warmup, 10), tuning_of(args), None,
                      peak_gbs, sm_max, False, kernels=False, warm_l2=True)
         warm = {"label": "warm L2: one plan, the same table every step (not the headline)", "plans_rotated": 1,
                 "ms_per_step": mw["ms_per_step"], "gupd_s": round(mw["gupd_s"], 1),
