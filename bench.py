@@ -444,6 +444,13 @@ def time_steps(rig, nsteps, warmup, dist=None, repeats=REPEATS):
             dist.barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
+        if rig.use_graph:
+            # device rigs: a ~30 us spin kernel in front of the first event keeps the stream busy while the host
+            # enqueues the graph launches, so that the events bracket the K steps' execution on the device and not the
+            # host's cudaGraphLaunch latency on an idle GPU (a 20-step region is ONE graph launch: ~10 us of it).  The
+            # host rig (e2e, direct calls) is timed without it: there the host's enqueue cost is part of the number.
+            with torch.cuda.stream(rig.stream):
+                torch.cuda._sleep(60000)
         e0.record(rig.stream)
         rig.run(nsteps)
         e1.record(rig.stream)
@@ -776,7 +783,8 @@ def run_ours(args):
                     "launch": "CUDA graph replay of pat_backproject (pre-pass + gather) per plan, graphs of <= %d "
                               "consecutive steps" % Rig.GRAPH_STEPS,
                     "timing": "median of %d regions of exactly `steps` steps each (CUDA events on the launching "
-                              "stream, max over ranks per region), after >= 2 full plan rotations of warm-up" % REPEATS,
+                              "stream, max over ranks per region; a 30 us spin kernel ahead of the first event hides the "
+                              "host's graph-launch latency), after >= 2 full plan rotations of warm-up" % REPEATS,
                     "regions_ms_per_step": main["regions_ms_per_step"],
                     "host_enqueue_us_per_direct_call": round(main["host_enqueue_us"], 2),
                     "host_enqueue_bursts_us": main["host_enqueue_bursts_us"]},
