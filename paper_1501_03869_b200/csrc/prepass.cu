@@ -228,53 +228,63 @@ constexpr int kB1Threads = 128, kB1U = 4;            // block size and quads per
 // (frame slot, sensor, quad) items are one flat index space -- the kernel above spends a 256-thread block on the 136
 // quads of one (frame, sensor) row of configs[1], 2048 of them at B = 4, and runs 2 - 3 blocks per SM beside three
 // resident gather CTAs: 5 - 7 waves of a load -> store round trip each -- small blocks (128 threads, <= 64 registers),
-// kB1U quads per thread a quarter of the grid apart, all loads issued before any is used.
+// kB1U quads per thread (the same quad of kB1U consecutive sensors), all loads issued before any is used.
 __global__ void __launch_bounds__(kB1Threads, 8)
 prepass_blocked_flat_kernel(const float *__restrict__ traces, float *__restrict__ b, float *__restrict__ images,
                             int32_t nsens, int32_t nt, int32_t ntb, int32_t nframes, int32_t log2_bp, int64_t nzero,
-                            float wp, float wd, float t0fs, int32_t n_lo, int32_t quads, uint32_t total, uint32_t *ready) {
+                            float wp, float wd, float t0fs, int32_t n_lo, int32_t quads, uint32_t total, uint32_t *ready,
+                            unsigned long long *trace) {
     asm volatile("griddepcontrol.launch_dependents;");
+    if (trace && threadIdx.x == 0) {
+        if (blockIdx.x == 0) trace[2] = pre_gtime();
+        if (blockIdx.x == gridDim.x - 1) trace[4] = pre_gtime();
+    }
     const uint32_t gid = blockIdx.x * kB1Threads + threadIdx.x, nthr = gridDim.x * kB1Threads;
     for (uint32_t q = gid; q < (uint32_t)nzero; q += nthr) images[q] = 0.0f;
-    const uint32_t per_frame = (uint32_t)nsens * (uint32_t)quads, bpm = (1u << log2_bp) - 1u;
-    for (uint32_t q = gid; q < total; q += kB1U * nthr) {
+    // an item = the same quad of kB1U consecutive sensors of one frame: its index arithmetic (two divisions, the
+    // interior test, the block address) is done once for four quads -- it was ~125 instructions per quad, 8.7 M warp
+    // instructions at 32 frames next to the gather's 48.7 M, and slowed the gather it runs beside by that much
+    const uint32_t ngrp = ((uint32_t)nsens + kB1U - 1u) / kB1U, per_frame = ngrp * (uint32_t)quads, bpm = (1u << log2_bp) - 1u;
+    const size_t row_out = ((size_t)ntb << log2_bp) * 32;                         // b: one sensor further
+    for (uint32_t q = gid; q < total; q += nthr) {
+        const uint32_t f = q / per_frame, r = q - f * per_frame, sg = r / (uint32_t)quads;
+        const int32_t n0 = n_lo + (int32_t)((r - sg * (uint32_t)quads) << 2);
+        const uint32_t s0 = sg * kB1U;
+        const bool live = f < (uint32_t)nframes && n0 < nt;                       // padding frames of the group, samples past the record: zeros
+        const float *p0 = traces + ((size_t)f * nsens + s0) * nt + n0;
         float w[kB1U][6];
-        uint32_t f[kB1U], srow[kB1U];
-        int32_t n0[kB1U];
 #pragma unroll
         for (int u = 0; u < kB1U; ++u) {
-            const uint32_t qq = min(q + u * nthr, total - 1u);                   // past the end: redo the last quad (harmless)
-            f[u] = qq / per_frame;
-            const uint32_t r = qq - f[u] * per_frame;
-            srow[u] = r / (uint32_t)quads;
-            n0[u] = n_lo + (int32_t)((r - srow[u] * (uint32_t)quads) << 2);
 #pragma unroll
             for (int j = 0; j < 6; ++j) w[u][j] = 0.0f;
-            if (f[u] < (uint32_t)nframes && n0[u] < nt) {                        // padding frames of the group, samples past the record: zeros
-                const float *p = traces + ((size_t)f[u] * nsens + srow[u]) * nt + n0[u];
+            if (live && s0 + u < (uint32_t)nsens) {
+                const float *p = p0 + (size_t)u * nt;
                 const float4 v = __ldg(reinterpret_cast<const float4 *>(p));
-                w[u][0] = n0[u] > 0 ? __ldg(p - 1) : 0.0f;
-                w[u][5] = n0[u] + 4 < nt ? __ldg(p + 4) : 0.0f;
+                w[u][0] = n0 > 0 ? __ldg(p - 1) : 0.0f;
+                w[u][5] = n0 + 4 < nt ? __ldg(p + 4) : 0.0f;
                 w[u][1] = v.x; w[u][2] = v.y; w[u][3] = v.z; w[u][4] = v.w;
             }
         }
+        const uint32_t g = f >> log2_bp, fl = f & bpm;
+        float *dst = b + ((((size_t)g * nsens + s0) * ntb + (uint32_t)(n0 >> 5)) << log2_bp) * 32 + (size_t)fl * 32 + (n0 & 31);
+        const bool interior = quad_interior(n0, nt, wd);
 #pragma unroll
         for (int u = 0; u < kB1U; ++u) {
+            if (s0 + u >= (uint32_t)nsens) break;
             float4 o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-            if (f[u] < (uint32_t)nframes && n0[u] < nt) {
-                if (quad_interior(n0[u], nt, wd)) {
-                    o = weight_quad_interior(w[u], n0[u], wp, t0fs);
+            if (live) {
+                if (interior) {
+                    o = weight_quad_interior(w[u], n0, wp, t0fs);
                 } else {
-                    o.x = weight_at(w[u] + 0, n0[u] + 0, nt, wp, wd, t0fs); o.y = weight_at(w[u] + 1, n0[u] + 1, nt, wp, wd, t0fs);
-                    o.z = weight_at(w[u] + 2, n0[u] + 2, nt, wp, wd, t0fs); o.w = weight_at(w[u] + 3, n0[u] + 3, nt, wp, wd, t0fs);
+                    o.x = weight_at(w[u] + 0, n0 + 0, nt, wp, wd, t0fs); o.y = weight_at(w[u] + 1, n0 + 1, nt, wp, wd, t0fs);
+                    o.z = weight_at(w[u] + 2, n0 + 2, nt, wp, wd, t0fs); o.w = weight_at(w[u] + 3, n0 + 3, nt, wp, wd, t0fs);
                 }
             }
-            const uint32_t g = f[u] >> log2_bp, fl = f[u] & bpm;
-            float *dst = b + ((((size_t)g * nsens + srow[u]) * ntb + (uint32_t)(n0[u] >> 5)) << log2_bp) * 32 + (size_t)fl * 32 + (n0[u] & 31);
-            *reinterpret_cast<float4 *>(dst) = o;
+            *reinterpret_cast<float4 *>(dst + (size_t)u * row_out) = o;
         }
     }
     prepass_block_done(ready);
+    if (trace && threadIdx.x == 0) atomicMax(trace + 3, pre_gtime());
 }
 
 // Bp = 16 (interleaved [sensor][sample][16], gather.cu PPL == 4).
@@ -626,12 +636,12 @@ int pat_launch_prepass(const PatLaunchCtx &ctx, const float *traces, float *b, f
     }
     if (blocked && (nt & 3) == 0 && !ctx.old_blocked_prepass) {
         const int32_t groups = (nframes + bp - 1) / bp;
-        const int64_t total = (int64_t)groups * bp * nsens * quads;
+        const int64_t total = (int64_t)groups * bp * ((nsens + kB1U - 1) / kB1U) * quads;     // items of kB1U quads
         if (total < (1ll << 31) && nzero < (1ll << 32)) {
-            int64_t nb = (total + kB1Threads * kB1U - 1) / (kB1Threads * kB1U);
+            int64_t nb = (total + kB1Threads - 1) / kB1Threads;
             if (nb > (int64_t)ctx.num_sms * 8) nb = (int64_t)ctx.num_sms * 8;
             return launch_pre(ctx, prepass_blocked_flat_kernel, dim3((unsigned)std::max<int64_t>(nb, 1)), kB1Threads, traces, b, images,
-                              nsens, nt, ntb, nframes, log2_bp, nzero, wp, wd, t0fs, n_lo, quads, (uint32_t)total, ready);
+                              nsens, nt, ntb, nframes, log2_bp, nzero, wp, wd, t0fs, n_lo, quads, (uint32_t)total, ready, ctx.pre_trace);
         }
     }
     if (blocked) {
