@@ -336,6 +336,17 @@ pat_status pat_eikonal_last_stats(int64_t *block_visits, int64_t *jacobi_iterati
 pat_status pat_compute_travel_times_gpu(pat_plan *plan, int32_t max_rounds, int32_t *rounds_out,
                                         void *stream);
 
+/* pat_pixel_order -- host only, no CUDA call: the slot order of the tile-major table pat_plan_create builds for this
+ * region.  perm_out[slot] = position in roi_index (0 .. npix-1), or -1 for the padding slots that fill the last tile;
+ * perm_out holds ceil(npix/256)*256 entries.  A tile is 256 consecutive slots, a warp of the gather takes 32 of them.
+ * The order is a recursive coordinate bisection (tiles, then halves down to groups of 8, Morton order inside), so that
+ * tiles and warps are spatially compact whatever the region's shape (a region that cuts the blocks of a plain Morton
+ * order -- the paper's "area within the skull", PAPER.md:79 -- would otherwise spread them over distant blocks);
+ * plain_morton != 0 gives round 1's plain Morton order (what PAT_PLAIN_MORTON=1 selects at plan creation).
+ * Errors: NULL / bad grid / index outside the grid -> PAT_ERR_INVALID_ARG. */
+pat_status pat_pixel_order(const pat_grid *grid, const int64_t *roi_index, int64_t npix, int32_t plain_morton,
+                           int32_t *perm_out);
+
 /* ---- the entry point that allocates nothing -------------------------------------------------------------
  * Eq. 7 with the sample-time weightings, for callers that cannot call cudaMalloc (code under CUDA
  * graph capture, tight serving loops, harnesses that forbid it): no plan, no workspace, no allocator.  The only

@@ -11,7 +11,7 @@ from .binding import (PAT_OK, PAT_ERR_INVALID_ARG, PAT_ERR_BAD_STATE, PAT_ERR_CU
                       pat_kernel_launches, pat_chained_calls, pat_set_device_allocator, pat_get_stats, install_torch_allocator,
                       torch_alloc, torch_free, PatStats, pat_set_gather_tuning, pat_fmm_travel_times,
                       pat_compute_travel_times, pat_set_profiling, pat_get_profile,
-                      pat_eikonal_travel_times_device, pat_eikonal_last_stats, pat_compute_travel_times_gpu,
+                      pat_eikonal_travel_times_device, pat_eikonal_last_stats, pat_pixel_order, pat_compute_travel_times_gpu,
                       pat_backproject_conventional, pat_backproject_conventional_sweep, pat_set_roi_mask, pat_set_pixel_weights,
                       pat_compute_solid_angle_weights, pat_get_trace_window, Plan,
                       pat_backproject_static, pat_backproject_static_max_samples, pat_backproject_static_last_error)

@@ -114,6 +114,8 @@ def lib():
                                                   ctypes.POINTER(i32), vp]
     L.pat_compute_travel_times_gpu.restype = ctypes.c_int
     L.pat_compute_travel_times_gpu.argtypes = [vp, i32, ctypes.POINTER(i32), vp]
+    L.pat_pixel_order.restype = ctypes.c_int
+    L.pat_pixel_order.argtypes = [gp, vp, i64, i32, vp]
     L.pat_eikonal_last_stats.restype = ctypes.c_int
     L.pat_eikonal_last_stats.argtypes = [ctypes.POINTER(i64)] * 3
     L.pat_backproject_static.restype = ctypes.c_int
@@ -344,6 +346,15 @@ def pat_eikonal_travel_times_device(grid, c_map, sensor_xyz, nsens, roi_index, n
     if st != PAT_OK:
         raise PatError(st, "pat_eikonal_travel_times_device failed")
     return r.value
+
+
+def pat_pixel_order(grid, roi_index, npix, plain_morton=False):
+    """Slot order of the tile-major table (host only): int32 array of ceil(npix/256)*256 entries, -1 = padding."""
+    out = np.empty(((int(npix) + 255) // 256) * 256, dtype=np.int32)
+    st = lib().pat_pixel_order(ctypes.byref(grid), _addr(roi_index), int(npix), 1 if plain_morton else 0, _addr(out))
+    if st != PAT_OK:
+        raise PatError(st, "pat_pixel_order")
+    return out
 
 
 def pat_eikonal_last_stats():

@@ -586,6 +586,95 @@ extern "C" size_t pat_plan_workspace_bytes(const pat_grid *grid, int32_t nsens, 
     return pat_layout(d).total;
 }
 
+// The order of the ROI pixels in the tile-major table (host only): slot -> ROI position, padded with -1 to whole tiles.
+// May throw std::bad_alloc.
+static std::vector<int32_t> build_pixel_order(const pat_grid *grid, const int64_t *roi_index, int64_t npix, bool plain_morton) {
+    const int64_t ntiles = (npix + kTilePix - 1) / kTilePix;
+    std::vector<int32_t> perm;
+    {
+        // spatially compact pixel order: sort ROI positions by the Morton key of their node
+        std::vector<uint64_t> key((size_t)npix);
+        const int64_t n0 = grid->n[0], n1 = grid->n[1];
+        for (int64_t j = 0; j < npix; ++j) {
+            const int64_t q = roi_index ? roi_index[j] : j;
+            const uint32_t ix = (uint32_t)(q % n0), iy = (uint32_t)((q / n0) % n1), iz = (uint32_t)(q / (n0 * n1));
+            key[j] = grid->ndim == 2 ? (spread2(ix) | (spread2(iy) << 1))
+                                     : (spread3(ix) | (spread3(iy) << 1) | (spread3(iz) << 2));
+        }
+        perm.assign((size_t)ntiles * kTilePix, -1);
+        std::iota(perm.begin(), perm.begin() + npix, 0);
+        std::sort(perm.begin(), perm.begin() + npix,
+                  [&](int32_t a, int32_t b) { return key[a] < key[b] || (key[a] == key[b] && a < b); });
+        // A tile of the gather is 256 consecutive slots and a warp takes 32 of them.  Plain Morton order is compact
+        // only where the region covers whole, ALIGNED blocks of the Morton grid: a disk (or a cube at an odd offset)
+        // cuts blocks, everything behind the first partial block is shifted, and a warp or a tile then straddles
+        // blocks that are neighbours on the Z-curve but not in space (configs[1]: 30 % of the warp rows span >= 32
+        // samples -- bank conflicts in the blocked trace layout -- and a tile's window is 90 samples on average, 268
+        // at the 99th percentile).  So the order is made by recursive coordinate bisection instead: split the pixel
+        // set at a multiple of 256 across the longest axis of its bounding box until the parts are tiles, then every
+        // tile the same way in halves down to groups of 8 (warps, half-warps and quarter-warps all compact; Morton order inside).  configs[1]: warp rows
+        // spanning >= 32 samples 0.1 %, windows 64 samples on average, 89 at the 99th percentile, 94 at most.
+        if (!plain_morton && npix > 32) {
+            const int nd = grid->ndim;
+            std::vector<int32_t> cx((size_t)npix), cy((size_t)npix), cz((size_t)npix);
+            for (int64_t j = 0; j < npix; ++j) {
+                const int64_t q = roi_index ? roi_index[j] : j;
+                cx[(size_t)j] = (int32_t)(q % n0); cy[(size_t)j] = (int32_t)((q / n0) % n1); cz[(size_t)j] = (int32_t)(q / (n0 * n1));
+            }
+            // iterative bisection of perm[lo, hi) into parts of `unit` slots (the last part may be shorter)
+            auto bisect = [&](int64_t lo0, int64_t hi0, int64_t unit) {
+                std::vector<std::pair<int64_t, int64_t>> todo{{lo0, hi0}};
+                while (!todo.empty()) {
+                    const auto [lo, hi] = todo.back();
+                    todo.pop_back();
+                    if (hi - lo <= unit) continue;
+                    int32_t mn[3] = {INT32_MAX, INT32_MAX, INT32_MAX}, mx[3] = {INT32_MIN, INT32_MIN, INT32_MIN};
+                    for (int64_t q = lo; q < hi; ++q) {
+                        const size_t a = (size_t)perm[(size_t)q];
+                        const int32_t c[3] = {cx[a], cy[a], cz[a]};
+                        for (int dd = 0; dd < nd; ++dd) { mn[dd] = std::min(mn[dd], c[dd]); mx[dd] = std::max(mx[dd], c[dd]); }
+                    }
+                    int ax = 0;
+                    for (int dd = 1; dd < nd; ++dd) if (mx[dd] - mn[dd] > mx[ax] - mn[ax]) ax = dd;
+                    const std::vector<int32_t> &co = ax == 0 ? cx : ax == 1 ? cy : cz;
+                    const int64_t units = (hi - lo + unit - 1) / unit, cut = lo + units / 2 * unit;
+                    std::nth_element(perm.begin() + lo, perm.begin() + cut, perm.begin() + hi, [&](int32_t a, int32_t b) {
+                        return co[(size_t)a] < co[(size_t)b] || (co[(size_t)a] == co[(size_t)b] && key[(size_t)a] < key[(size_t)b]);
+                    });
+                    todo.push_back({lo, cut});
+                    todo.push_back({cut, hi});
+                }
+            };
+            bisect(0, npix, kTilePix);
+            for (int64_t t0 = 0; t0 < npix; t0 += kTilePix) {
+                const int64_t t1 = std::min<int64_t>(npix, t0 + kTilePix);
+                bisect(t0, t1, 8);       // halves all the way down: 128, 64, 32 (a warp), 16 (a half-warp: 64-bit loads), 8
+                for (int64_t w0 = t0; w0 < t1; w0 += 8)
+                    std::sort(perm.begin() + w0, perm.begin() + std::min<int64_t>(t1, w0 + 8),
+                              [&](int32_t a, int32_t b) { return key[(size_t)a] < key[(size_t)b]; });
+            }
+            // tiles in the Morton order of their first pixel: consecutive tiles (consecutive CTAs' shares) stay neighbours
+            const int64_t nt_full = (npix + kTilePix - 1) / kTilePix;
+            std::vector<int64_t> tord((size_t)nt_full);
+            std::iota(tord.begin(), tord.end(), 0);
+            auto tile_key = [&](int64_t t) {
+                uint64_t m = ~0ull;
+                for (int64_t q = t * kTilePix; q < std::min<int64_t>(npix, (t + 1) * kTilePix); ++q) m = std::min(m, key[(size_t)perm[(size_t)q]]);
+                return m;
+            };
+            std::vector<uint64_t> tk((size_t)nt_full);
+            for (int64_t t = 0; t < nt_full; ++t) tk[(size_t)t] = tile_key(t);
+            // the short last tile stays last (its padding lanes end the slot array)
+            std::sort(tord.begin(), tord.end() - ((npix % kTilePix) ? 1 : 0), [&](int64_t a, int64_t b) { return tk[(size_t)a] < tk[(size_t)b]; });
+            std::vector<int32_t> tmp(perm.begin(), perm.begin() + npix);
+            int64_t w = 0;
+            for (int64_t t : tord)
+                for (int64_t q = t * kTilePix; q < std::min<int64_t>(npix, (t + 1) * kTilePix); ++q) perm[(size_t)w++] = tmp[(size_t)q];
+        }
+    }
+    return perm;
+}
+
 extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, const float *c_map,
                                       const float *sensor_xyz, int32_t nsens,
                                       const int64_t *roi_index, int64_t npix,
@@ -668,85 +757,7 @@ extern "C" pat_status pat_plan_create(pat_plan **out, const pat_grid *grid, cons
         if (c_map) p->c_map.assign(c_map, c_map + N);
         if (sensor_xyz) p->sensors.assign(sensor_xyz, sensor_xyz + (int64_t)nsens * 3);
         if (roi_index) p->roi.assign(roi_index, roi_index + npix);
-        // spatially compact pixel order: sort ROI positions by the Morton key of their node
-        std::vector<uint64_t> key((size_t)npix);
-        const int64_t n0 = grid->n[0], n1 = grid->n[1];
-        for (int64_t j = 0; j < npix; ++j) {
-            const int64_t q = roi_index ? roi_index[j] : j;
-            const uint32_t ix = (uint32_t)(q % n0), iy = (uint32_t)((q / n0) % n1), iz = (uint32_t)(q / (n0 * n1));
-            key[j] = grid->ndim == 2 ? (spread2(ix) | (spread2(iy) << 1))
-                                     : (spread3(ix) | (spread3(iy) << 1) | (spread3(iz) << 2));
-        }
-        perm.assign((size_t)p->dims.ntiles * kTilePix, -1);
-        std::iota(perm.begin(), perm.begin() + npix, 0);
-        std::sort(perm.begin(), perm.begin() + npix,
-                  [&](int32_t a, int32_t b) { return key[a] < key[b] || (key[a] == key[b] && a < b); });
-        // A tile of the gather is 256 consecutive slots and a warp takes 32 of them.  Plain Morton order is compact
-        // only where the region covers whole, ALIGNED blocks of the Morton grid: a disk (or a cube at an odd offset)
-        // cuts blocks, everything behind the first partial block is shifted, and a warp or a tile then straddles
-        // blocks that are neighbours on the Z-curve but not in space (configs[1]: 30 % of the warp rows span >= 32
-        // samples -- bank conflicts in the blocked trace layout -- and a tile's window is 90 samples on average, 268
-        // at the 99th percentile).  So the order is made by recursive coordinate bisection instead: split the pixel
-        // set at a multiple of 256 across the longest axis of its bounding box until the parts are tiles, then every
-        // tile the same way in halves down to groups of 8 (warps, half-warps and quarter-warps all compact; Morton order inside).  configs[1]: warp rows
-        // spanning >= 32 samples 0.1 %, windows 64 samples on average, 89 at the 99th percentile, 94 at most.
-        if (std::getenv("PAT_PLAIN_MORTON") == nullptr && npix > 32) {
-            const int nd = grid->ndim;
-            std::vector<int32_t> cx((size_t)npix), cy((size_t)npix), cz((size_t)npix);
-            for (int64_t j = 0; j < npix; ++j) {
-                const int64_t q = roi_index ? roi_index[j] : j;
-                cx[(size_t)j] = (int32_t)(q % n0); cy[(size_t)j] = (int32_t)((q / n0) % n1); cz[(size_t)j] = (int32_t)(q / (n0 * n1));
-            }
-            // iterative bisection of perm[lo, hi) into parts of `unit` slots (the last part may be shorter)
-            auto bisect = [&](int64_t lo0, int64_t hi0, int64_t unit) {
-                std::vector<std::pair<int64_t, int64_t>> todo{{lo0, hi0}};
-                while (!todo.empty()) {
-                    const auto [lo, hi] = todo.back();
-                    todo.pop_back();
-                    if (hi - lo <= unit) continue;
-                    int32_t mn[3] = {INT32_MAX, INT32_MAX, INT32_MAX}, mx[3] = {INT32_MIN, INT32_MIN, INT32_MIN};
-                    for (int64_t q = lo; q < hi; ++q) {
-                        const size_t a = (size_t)perm[(size_t)q];
-                        const int32_t c[3] = {cx[a], cy[a], cz[a]};
-                        for (int dd = 0; dd < nd; ++dd) { mn[dd] = std::min(mn[dd], c[dd]); mx[dd] = std::max(mx[dd], c[dd]); }
-                    }
-                    int ax = 0;
-                    for (int dd = 1; dd < nd; ++dd) if (mx[dd] - mn[dd] > mx[ax] - mn[ax]) ax = dd;
-                    const std::vector<int32_t> &co = ax == 0 ? cx : ax == 1 ? cy : cz;
-                    const int64_t units = (hi - lo + unit - 1) / unit, cut = lo + units / 2 * unit;
-                    std::nth_element(perm.begin() + lo, perm.begin() + cut, perm.begin() + hi, [&](int32_t a, int32_t b) {
-                        return co[(size_t)a] < co[(size_t)b] || (co[(size_t)a] == co[(size_t)b] && key[(size_t)a] < key[(size_t)b]);
-                    });
-                    todo.push_back({lo, cut});
-                    todo.push_back({cut, hi});
-                }
-            };
-            bisect(0, npix, kTilePix);
-            for (int64_t t0 = 0; t0 < npix; t0 += kTilePix) {
-                const int64_t t1 = std::min<int64_t>(npix, t0 + kTilePix);
-                bisect(t0, t1, 8);       // halves all the way down: 128, 64, 32 (a warp), 16 (a half-warp: 64-bit loads), 8
-                for (int64_t w0 = t0; w0 < t1; w0 += 8)
-                    std::sort(perm.begin() + w0, perm.begin() + std::min<int64_t>(t1, w0 + 8),
-                              [&](int32_t a, int32_t b) { return key[(size_t)a] < key[(size_t)b]; });
-            }
-            // tiles in the Morton order of their first pixel: consecutive tiles (consecutive CTAs' shares) stay neighbours
-            const int64_t nt_full = (npix + kTilePix - 1) / kTilePix;
-            std::vector<int64_t> tord((size_t)nt_full);
-            std::iota(tord.begin(), tord.end(), 0);
-            auto tile_key = [&](int64_t t) {
-                uint64_t m = ~0ull;
-                for (int64_t q = t * kTilePix; q < std::min<int64_t>(npix, (t + 1) * kTilePix); ++q) m = std::min(m, key[(size_t)perm[(size_t)q]]);
-                return m;
-            };
-            std::vector<uint64_t> tk((size_t)nt_full);
-            for (int64_t t = 0; t < nt_full; ++t) tk[(size_t)t] = tile_key(t);
-            // the short last tile stays last (its padding lanes end the slot array)
-            std::sort(tord.begin(), tord.end() - ((npix % kTilePix) ? 1 : 0), [&](int64_t a, int64_t b) { return tk[(size_t)a] < tk[(size_t)b]; });
-            std::vector<int32_t> tmp(perm.begin(), perm.begin() + npix);
-            int64_t w = 0;
-            for (int64_t t : tord)
-                for (int64_t q = t * kTilePix; q < std::min<int64_t>(npix, (t + 1) * kTilePix); ++q) perm[(size_t)w++] = tmp[(size_t)q];
-        }
+        perm = build_pixel_order(grid, roi_index, npix, std::getenv("PAT_PLAIN_MORTON") != nullptr);
     } catch (...) {
         delete p;
         return fail(nullptr, PAT_ERR_NOMEM, "host allocation failed");
@@ -1317,5 +1328,24 @@ extern "C" pat_status pat_set_roi_mask(pat_plan *p, const uint8_t *mask) {
     }
     e = cudaMemcpy(p->d_perm_masked, perm.data(), (size_t)slots * sizeof(int32_t), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) return cuda_fail(p, e, "roi mask upload");
+    return PAT_OK;
+}
+
+// Host only (no CUDA call): the slot order pat_plan_create would use for this region -- for tests of the order's
+// properties and for callers that want to lay out their own per-pixel data tile-major.
+extern "C" pat_status pat_pixel_order(const pat_grid *grid, const int64_t *roi_index, int64_t npix, int32_t plain_morton,
+                                      int32_t *perm_out) {
+    if (!grid || !perm_out || npix <= 0 || npix > (int64_t)INT32_MAX) return PAT_ERR_INVALID_ARG;
+    if (grid->ndim != 2 && grid->ndim != 3) return PAT_ERR_INVALID_ARG;
+    int64_t N = 1;
+    for (int dd = 0; dd < grid->ndim; ++dd) { if (grid->n[dd] < 1) return PAT_ERR_INVALID_ARG; N *= grid->n[dd]; }
+    if (!roi_index && npix != N) return PAT_ERR_INVALID_ARG;
+    if (roi_index)
+        for (int64_t j = 0; j < npix; ++j)
+            if (roi_index[j] < 0 || roi_index[j] >= N) return PAT_ERR_INVALID_ARG;
+    try {
+        const std::vector<int32_t> perm = build_pixel_order(grid, roi_index, npix, plain_morton != 0);
+        std::copy(perm.begin(), perm.end(), perm_out);
+    } catch (...) { return PAT_ERR_NOMEM; }
     return PAT_OK;
 }

@@ -169,3 +169,38 @@ def test_device_allocator_abi_without_a_gpu():
     assert L.pat_set_device_allocator(ctypes.cast(cb, ctypes.c_void_p), None, None) == pat.PAT_ERR_INVALID_ARG
     assert L.pat_set_device_allocator(None, None, None) == pat.PAT_OK
     assert L.pat_get_stats(None, None) == pat.PAT_ERR_INVALID_ARG
+
+
+def _extents(perm, roi, n, group):
+    """Largest bounding-box edge (nodes) of every `group` consecutive slots of the order."""
+    pos = perm[perm >= 0]
+    q = roi[pos]
+    co = [q % n[0], (q // n[0]) % n[1]] + ([q // (n[0] * n[1])] if len(n) == 3 else [])
+    out = []
+    for a in range(0, len(pos), group):
+        out.append(max(int(c[a:a + group].max() - c[a:a + group].min()) for c in co))
+    return np.array(out)
+
+
+def test_pixel_order_is_a_compact_permutation_2d_disk_and_3d_offset_cube():
+    """Host logic of the table layout (pat_pixel_order = what pat_plan_create uses): a bijection with the padding at
+    the end, and spatially compact tiles (256 slots) and warps (32 slots) for regions that cut the blocks of a plain
+    Morton order -- the paper's region within the skull (configs[1]: a disk of 21323 nodes) and a cube at an odd
+    offset inside a larger grid (configs[4] reduced) -- where plain Morton order is NOT compact."""
+    for k, reduced, tile_max, warp_max in [(1, False, 30, 13), (4, True, 9, 4)]:
+        geom = W.make_geometry(k, reduced)
+        grid = pat.PatGrid.make(geom.n, geom.h, geom.origin)
+        roi = np.ascontiguousarray(geom.roi_index, dtype=np.int64)
+        P = geom.npix
+        perm = pat.pat_pixel_order(grid, roi, P)
+        assert perm.shape == (((P + 255) // 256) * 256,)
+        assert np.array_equal(np.sort(perm[:P]), np.arange(P)) and (perm[P:] == -1).all()
+        tiles, warps = _extents(perm, roi, geom.n, 256), _extents(perm, roi, geom.n, 32)
+        assert tiles.max() <= tile_max and warps.max() <= warp_max, (k, tiles.max(), warps.max())
+        plain = pat.pat_pixel_order(grid, roi, P, plain_morton=True)
+        assert np.array_equal(np.sort(plain[:P]), np.arange(P))
+        assert _extents(plain, roi, geom.n, 32).max() > 2 * warp_max        # what the bisection order is for
+    g = pat.PatGrid.make((8, 8), 1e-3, (0, 0))
+    with pytest.raises(pat.PatError):
+        pat.pat_pixel_order(g, np.array([0, 64], dtype=np.int64), 2)       # index outside the grid
+    assert np.array_equal(np.sort(pat.pat_pixel_order(g, None, 64)[:64]), np.arange(64))
