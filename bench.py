@@ -439,9 +439,9 @@ def time_steps(rig, nsteps, warmup, dist=None, repeats=REPEATS):
     rig.run(nsteps)
     torch.cuda.synchronize()
     regions = []
-    for _ in range(repeats):
-        if dist is not None:
-            dist.barrier()
+    for rep in range(-2, repeats):                       # two dress rehearsals of the same structure first (not recorded):
+        if dist is not None:                             # the first regions after the warm-up run 10 - 50 % long (lazy loading
+            dist.barrier()                               # of the spin kernel, clocks and L2 state after the synchronize)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
         if rig.use_graph:
@@ -459,7 +459,8 @@ def time_steps(rig, nsteps, warmup, dist=None, repeats=REPEATS):
         if dist is not None:
             ms = max_over_ranks(ms, dist, device="cuda")
             dist.barrier()
-        regions.append(ms)
+        if rep >= 0:
+            regions.append(ms)
     rig.last_regions = regions
     return float(np.median(regions))
 
